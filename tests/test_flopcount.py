@@ -1,0 +1,24 @@
+"""The contract flop count is produced by oracle/flopcount (counting scalar type run through
+the oracle's own per-point routines).  Check it runs and sits where the survey's hand count (±15 %) put it."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_flopcount_runs_and_matches_hand_count():
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import build
+
+    build.build()
+    out = json.loads(subprocess.check_output([os.path.join(ROOT, "oracle", "flopcount")]))
+    ns = out["total_navier_stokes_per_point_stage"]["total"]
+    eu = out["total_euler_per_point_stage"]["total"]
+    assert 0.85 * 4200 < ns < 1.15 * 4200 * 1.0 + 400  # survey hand count ~4.2 kflop (N-S)
+    assert 0.85 * 3800 < eu < 1.15 * 3800
+    s2 = out["S2_per_direction_modified"]
+    assert s2["sqrt"] >= 6 and s2["div"] >= 32
+    # the paper's claim for the modified scheme: sharing beta and the characteristic variables "reduces calculation"
+    assert out["S2_per_direction_original"]["total"] > 1.3 * s2["total"]
