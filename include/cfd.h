@@ -1,0 +1,145 @@
+/* =====================================================================================
+ * cfd.h — C ABI of the B200-native (sm_100a) fp64 hot path of
+ *   Ye, Zhang, Wan, Yan, Sun, "Accelerating CFD simulation with high order finite difference
+ *   method on curvilinear coordinates for modern GPU clusters", Adv. Aerodyn. 4:7 (2022).
+ * Citations: P:L<n> = line n of /root/reference/PAPER.md; U<k> = reading k in DESIGN.md §3.
+ *
+ * The path: right-hand side R(Q) of the compressible Navier–Stokes equations in strong
+ * conservation form on curvilinear multi-block structured grids (Eq. 2) and the
+ * TVD-RK3 stage update (Eq. 20), in the stage order of Fig. 2:
+ *     cfd_rhs -> cfd_rk_stage -> cfd_exchange_interfaces -> cfd_apply_bc .
+ *
+ * General rules
+ *  - Every function returns 0 (CFD_OK) on success and a negative cfd_status on error; nothing
+ *    throws, nothing calls exit().  cfd_last_error() returns a message for the last failure.
+ *  - All field buffers are DEVICE pointers OWNED BY THE CALLER (e.g. torch tensors) for the
+ *    whole life of the context; the library keeps non-owning pointers and never frees them.
+ *  - Layout of every field: fp64, structure-of-arrays [var][k][j][i], i fastest, each axis
+ *    carrying CFD_NG = 6 ghost layers on both sides: extents (ni+12, nj+12, nk+12),
+ *    M = (ni+12)(nj+12)(nk+12) doubles per variable.  Pointers must be 16-byte aligned.
+ *  - All work is enqueued on the CUDA stream given to cfd_create_blocks; no function
+ *    synchronises the device unless documented ("returns host values").
+ *  - No cudaMalloc/cudaFree after cfd_create_blocks (which allocates a few KB of descriptors).
+ *  - There is no CPU fallback: without a CUDA device cfd_create_blocks fails with CFD_E_CUDA.
+ * ===================================================================================== */
+#ifndef CFD_B200_H
+#define CFD_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CFD_NG 6 /* ghost layers per face (U12; the paper has ghost cells, M != N, depth unstated) */
+
+typedef enum {
+  CFD_OK = 0,
+  CFD_E_ARG = -1,       /* null / misaligned pointer, bad size, bad enum */
+  CFD_E_TOPOLOGY = -2,  /* inconsistent face descriptor (perm/sign/extents) */
+  CFD_E_JACOBIAN = -3,  /* J <= 0 at an interior node (cfd_compute_metrics) */
+  CFD_E_STAGE = -4,     /* RK stage not in 1..3 */
+  CFD_E_WORKSPACE = -5, /* workspace too small / null */
+  CFD_E_CUDA = -6       /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+} cfd_status;
+
+/* face types (S5/S6; the paper names bc_block / bc_phys only) */
+#define CFD_FACE_PERIODIC 1
+#define CFD_FACE_INTERFACE 2
+#define CFD_FACE_WALL_NOSLIP_ADIABATIC 3 /* U13 */
+#define CFD_FACE_FARFIELD_CHAR 4         /* U14 */
+
+typedef struct cfd_ctx cfd_ctx; /* opaque, owned by the library */
+
+typedef struct {
+  int ni, nj, nk; /* interior sizes (>= 6 each); arrays are (n + 2*CFD_NG) per axis */
+} cfd_dims;
+
+typedef struct {
+  double gamma;    /* ratio of specific heats (1.4 in the paper) */
+  double mach;     /* Ma_inf  (viscous scaling Ma/Re of tau and q) */
+  double reynolds; /* Re_inf */
+  double prandtl;  /* Pr */
+  double weno_eps; /* epsilon of Eq. 15 (1e-6) */
+  int viscous;     /* 0 Euler, 1 Navier–Stokes with constant mu = 1 (U11) */
+  int scheme;      /* 0 modified AFWENO (Fig. 11); 1 original (Fig. 9) */
+  double q_inf[5]; /* far-field conservative state (rho, rho u, rho v, rho w, e) */
+} cfd_params;
+
+typedef struct {
+  int block, face;         /* face: 0 -xi, 1 +xi, 2 -eta, 3 +eta, 4 -zeta, 5 +zeta */
+  int type;                /* CFD_FACE_* */
+  int nbr_block, nbr_face; /* PERIODIC / INTERFACE only */
+  int perm[3];             /* my axis a runs along the neighbour's axis perm[a] ... */
+  int sign[3];             /* ... in direction sign[a] = +1 / -1 (proper rotations only) */
+  double shift[3];         /* (x,y,z) translation added to the neighbour's coordinates when they
+                              become my ghost coordinates (periodic images) */
+} cfd_face;
+
+typedef struct {
+  double* q;    /* [5][M] conservative variables Q = (rho, rho u, rho v, rho w, e), no 1/J */
+  double* qn;   /* [5][M] Q^n of Eq. 20 */
+  double* r;    /* [5][M] R(Q) */
+  double* xyz;  /* [3][M] node coordinates; the caller fills the interior, the library the ghosts */
+  double* khat; /* [9][M] hatted metrics, index d*3+c = d(xi^d)/d(x_c) / J  (Eq. 7) */
+  double* jac;  /* [1][M] J (Eq. 8) */
+} cfd_block_ptrs;
+
+/* Bytes of device scratch the caller must pass to cfd_create_blocks (12 doubles per point of the
+ * largest block: viscous point fluxes / metric first derivatives, plus reduction partials). */
+size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params* params);
+
+/* Build a context over nblocks point-matched blocks (a patch is a whole block face).
+ * Validates sizes, alignment and the face descriptors (permutation proper, normal-axis sign
+ * consistent with the face pair, tangential extents equal).  `workspace` is device memory of at
+ * least cfd_workspace_bytes(), caller-owned.  `cuda_stream` is a cudaStream_t (may be 0). */
+int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cfd_block_ptrs* ptrs, int nfaces,
+                      const cfd_face* faces, const cfd_params* params, void* workspace, size_t workspace_bytes,
+                      void* cuda_stream);
+
+/* S1 (Eqs. 7–8): fills the ghost layers of xyz (interfaces / periodic shift, wall = odd
+ * reflection, far field = linear extrapolation), then khat and jac by 6th-order central differences
+ * in conservative form, valid on the index box [-3, n+3)^3 of every block.
+ * Returns host values: synchronises the stream; CFD_E_JACOBIAN if J <= 0 at an interior node. */
+int cfd_compute_metrics(cfd_ctx*);
+
+/* S2 + S3 (Eqs. 9–19 with Steger–Warming splitting and the modified AFWENO of Fig. 11; Eqs. 5, 6, 21
+ * with 6th-order central differences): r := J [ sum_d d(Fv^d)/d(xi^d) - sum_d D^d ] on interior points.
+ * Requires valid ghost layers in q (cfd_exchange_interfaces + cfd_apply_bc).  Asynchronous. */
+int cfd_rhs(cfd_ctx*);
+
+/* S4 (Eq. 20): q <- a q^n + b (q + dt r) on interior points, (a,b) = (0,1), (3/4,1/4), (1/3,2/3) for
+ * stage 1, 2, 3; stage 1 first saves q^n := q and accumulates res_m = sum over all blocks' interior
+ * points of r_m^2 with a fixed-order (run-to-run deterministic) reduction.
+ * res5_host_or_null: if non-null (stage 1 only) receives the 5 sums and the stream is synchronised. */
+int cfd_rk_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
+
+/* S6: fills the ghost layers of q behind PERIODIC / INTERFACE faces from the
+ * neighbour's interior through the signed index permutation, faces then edges then corners. */
+int cfd_exchange_interfaces(cfd_ctx*);
+
+/* S5: no-slip adiabatic wall (U13) and characteristic far field (U14) on q: boundary
+ * node plane and the 6 ghost layers behind it, tangential index range [-3, n+3). */
+int cfd_apply_bc(cfd_ctx*);
+
+/* Convenience: the four calls above for one stage, in Fig. 2's order, on the context's stream. */
+int cfd_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
+
+/* Frees the context (never the caller's buffers). */
+int cfd_destroy(cfd_ctx*);
+
+/* Message for the most recent failing call on this context (or on creation if ctx == NULL). */
+const char* cfd_last_error(const cfd_ctx*);
+
+/* Number of kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
+long long cfd_launch_count(const cfd_ctx*);
+
+/* Register-resident DFMA loop on the context-free default stream: measures the plain FP64 FMA
+ * throughput of the device (the "alu" roofline denominator).  Returns host values (TFLOP/s,
+ * FMA = 2 flops) in *tflops; synchronises. */
+int cfd_fp64_peak_probe(int iters, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CFD_B200_H */

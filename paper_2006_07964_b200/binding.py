@@ -1,0 +1,201 @@
+"""Thin ctypes binding of the C ABI in include/cfd.h (argument marshalling only).
+
+PyTorch is used for device memory and the CUDA stream — plumbing, not the product: every step of
+the path runs in the kernels of csrc/.  There is NO CPU fallback: importing this module raises if
+libcfd_b200.so is missing, and `Context` raises if there is no CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+NG = 6
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcfd_b200.so")
+
+ABI_SYMBOLS = (
+    "cfd_workspace_bytes", "cfd_create_blocks", "cfd_compute_metrics", "cfd_rhs", "cfd_rk_stage",
+    "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
+    "cfd_launch_count", "cfd_fp64_peak_probe",
+)
+
+
+class CfdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"cfd error {code}: {msg}")
+        self.code = code
+
+
+class _Dims(C.Structure):
+    _fields_ = [("ni", C.c_int), ("nj", C.c_int), ("nk", C.c_int)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("mach", C.c_double), ("reynolds", C.c_double), ("prandtl", C.c_double),
+                ("weno_eps", C.c_double), ("viscous", C.c_int), ("scheme", C.c_int), ("q_inf", C.c_double * 5)]
+
+
+class _Face(C.Structure):
+    _fields_ = [("block", C.c_int), ("face", C.c_int), ("type", C.c_int), ("nbr_block", C.c_int),
+                ("nbr_face", C.c_int), ("perm", C.c_int * 3), ("sign", C.c_int * 3), ("shift", C.c_double * 3)]
+
+
+class _Ptrs(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("q", "qn", "r", "xyz", "khat", "jac")]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2006_07964_b200.build` "
+            "(nvcc, sm_100a). There is no CPU fallback for this library.")
+    L = C.CDLL(LIB_PATH)
+    L.cfd_workspace_bytes.restype = C.c_size_t
+    L.cfd_workspace_bytes.argtypes = [C.c_int, C.POINTER(_Dims), C.POINTER(_Params)]
+    L.cfd_create_blocks.restype = C.c_int
+    L.cfd_create_blocks.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(_Dims), C.POINTER(_Ptrs), C.c_int,
+                                    C.POINTER(_Face), C.POINTER(_Params), C.c_void_p, C.c_size_t, C.c_void_p]
+    for n in ("cfd_compute_metrics", "cfd_rhs", "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_destroy"):
+        getattr(L, n).restype = C.c_int
+        getattr(L, n).argtypes = [C.c_void_p]
+    for n in ("cfd_rk_stage", "cfd_stage"):
+        getattr(L, n).restype = C.c_int
+        getattr(L, n).argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_double)]
+    L.cfd_last_error.restype = C.c_char_p
+    L.cfd_last_error.argtypes = [C.c_void_p]
+    L.cfd_launch_count.restype = C.c_longlong
+    L.cfd_launch_count.argtypes = [C.c_void_p]
+    L.cfd_fp64_peak_probe.restype = C.c_int
+    L.cfd_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    return L
+
+
+lib = _load()
+
+
+def device_peak_probe(iters=4096):
+    """Measured FP64 FMA throughput of the current device in TFLOP/s (FMA = 2 flops)."""
+    t = C.c_double()
+    rc = lib.cfd_fp64_peak_probe(int(iters), C.byref(t))
+    if rc != 0:
+        raise CfdError(rc, "cfd_fp64_peak_probe failed")
+    return t.value
+
+
+class Context:
+    """One solver context over `dims` blocks.  Allocates the device fields with torch (fp64,
+    [var][k][j][i] with 6 ghost layers) and hands raw pointers to the C ABI."""
+
+    NV = dict(q=5, qn=5, r=5, xyz=3, khat=9, jac=1)
+
+    def __init__(self, dims, faces, params, device="cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise CfdError(-6, "no CUDA device: this library has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.dims = [tuple(int(x) for x in d) for d in dims]
+        nb = len(self.dims)
+        self.fields = []
+        with torch.cuda.device(self.device):
+            for (ni, nj, nk) in self.dims:
+                shp = (nk + 2 * NG, nj + 2 * NG, ni + 2 * NG)
+                self.fields.append({n: torch.zeros((nv,) + shp, dtype=torch.float64, device=self.device)
+                                    for n, nv in self.NV.items()})
+            d = (_Dims * nb)(*[_Dims(*dd) for dd in self.dims])
+            p = _Params()
+            for k in ("gamma", "mach", "reynolds", "prandtl", "weno_eps", "viscous", "scheme"):
+                setattr(p, k, params[k])
+            for a in range(5):
+                p.q_inf[a] = params["q_inf"][a]
+            fa = (_Face * max(1, len(faces)))()
+            for t, f in enumerate(faces):
+                fa[t].block, fa[t].face, fa[t].type = f["block"], f["face"], f["type"]
+                fa[t].nbr_block, fa[t].nbr_face = f["nbr_block"], f["nbr_face"]
+                for a in range(3):
+                    fa[t].perm[a], fa[t].sign[a], fa[t].shift[a] = f["perm"][a], f["sign"][a], f["shift"][a]
+            ptrs = (_Ptrs * nb)()
+            for b in range(nb):
+                for n in self.NV:
+                    setattr(ptrs[b], n, self.fields[b][n].data_ptr())
+            wsb = lib.cfd_workspace_bytes(nb, d, C.byref(p))
+            self.workspace = torch.empty((wsb + 7) // 8, dtype=torch.float64, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            rc = lib.cfd_create_blocks(C.byref(h), nb, d, ptrs, len(faces), fa, C.byref(p), self.workspace.data_ptr(),
+                                       wsb, C.c_void_p(self.stream.cuda_stream))
+            if rc != 0:
+                raise CfdError(rc, lib.cfd_last_error(None).decode())
+            self.h = h
+
+    # ---- lifetime ----
+    def close(self):
+        if getattr(self, "h", None):
+            lib.cfd_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc):
+        if rc != 0:
+            raise CfdError(rc, lib.cfd_last_error(self.h).decode())
+
+    # ---- data movement helpers (harness side) ----
+    def interior(self, b, name):
+        return self.fields[b][name][:, NG:-NG, NG:-NG, NG:-NG]
+
+    def load_case(self, case):
+        t = self.torch
+        for b in range(len(self.dims)):
+            self.interior(b, "xyz").copy_(t.from_numpy(np.ascontiguousarray(case.xyz[b])))
+            self.interior(b, "q").copy_(t.from_numpy(np.ascontiguousarray(case.q0[b])))
+        self.compute_metrics()
+        self.exchange_interfaces()
+        self.apply_bc()
+
+    def to_numpy(self, b, name, interior=True):
+        a = self.interior(b, name) if interior else self.fields[b][name]
+        return a.detach().cpu().numpy()
+
+    # ---- the C ABI, same names ----
+    def compute_metrics(self):
+        self._chk(lib.cfd_compute_metrics(self.h))
+
+    def rhs(self):
+        self._chk(lib.cfd_rhs(self.h))
+
+    def rk_stage(self, stage, dt, want_res=False):
+        res = (C.c_double * 5)()
+        self._chk(lib.cfd_rk_stage(self.h, int(stage), float(dt), res if want_res else None))
+        return np.array(res[:]) if want_res else None
+
+    def exchange_interfaces(self):
+        self._chk(lib.cfd_exchange_interfaces(self.h))
+
+    def apply_bc(self):
+        self._chk(lib.cfd_apply_bc(self.h))
+
+    def stage(self, stage, dt, want_res=False):
+        res = (C.c_double * 5)()
+        self._chk(lib.cfd_stage(self.h, int(stage), float(dt), res if want_res else None))
+        return np.array(res[:]) if want_res else None
+
+    def step(self, dt, want_res=False):
+        """One TVD-RK3 step = three stages in the order of Fig. 2."""
+        res = None
+        for s in (1, 2, 3):
+            r = self.stage(s, dt, want_res=(want_res and s == 1))
+            if s == 1:
+                res = r
+        return res
+
+    @property
+    def launch_count(self):
+        return int(lib.cfd_launch_count(self.h))

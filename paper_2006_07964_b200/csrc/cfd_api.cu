@@ -1,0 +1,248 @@
+// C-ABI entry points (include/cfd.h): validation, host-side topology planning, launch sequencing.
+// Every step of the path itself runs in the kernels of k_*.cu.
+#include <cstdint>
+#include <cstring>
+
+#include "cfd_internal.cuh"
+
+static thread_local std::string g_create_err;
+
+static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD_FACE_INTERFACE; }
+
+size_t ws_partials_offset_doubles(long long max_M) { return (size_t)12 * (size_t)max_M; }
+int rk_max_partial_blocks() { return 4096; }
+
+extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
+  long long mx = 0;
+  for (int b = 0; b < nblocks; ++b) {
+    long long M = (long long)(dims[b].ni + 2 * NG) * (dims[b].nj + 2 * NG) * (dims[b].nk + 2 * NG);
+    if (M > mx) mx = M;
+  }
+  return (ws_partials_offset_doubles(mx) + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
+}
+
+static int fail_create(int code, const std::string& msg) {
+  g_create_err = msg;
+  return code;
+}
+
+// Host-side plan of the ghost fill (U15): 26 regions per block, each filled through the lowest axis
+// whose face is PERIODIC/INTERFACE; pass = number of out-of-range indices (faces, edges, corners).
+static void plan_copies(cfd_ctx* c) {
+  for (size_t b = 0; b < c->blk.size(); ++b) {
+    const BlockDev& B = c->blk[b];
+    int ftype[6], fidx[6];
+    for (int s = 0; s < 6; ++s) { ftype[s] = 0; fidx[s] = -1; }
+    for (size_t t = 0; t < c->faces.size(); ++t)
+      if (c->faces[t].block == (int)b) { ftype[c->faces[t].face] = c->faces[t].type; fidx[c->faces[t].face] = (int)t; }
+    for (int code = 0; code < 27; ++code) {
+      int side[3] = {code % 3, (code / 3) % 3, code / 9};  // 0 below, 1 inside, 2 above
+      int nout = 0, fsel = -1;
+      for (int a = 0; a < 3; ++a) {
+        if (side[a] == 1) continue;
+        ++nout;
+        int fc = 2 * a + (side[a] == 2 ? 1 : 0);
+        if (fsel < 0 && is_connect(ftype[fc])) fsel = fc;
+      }
+      if (nout == 0 || fsel < 0) continue;
+      const cfd_face& F = c->faces[fidx[fsel]];
+      const BlockDev& N = c->blk[F.nbr_block];
+      CopyTask T;
+      T.dst_block = (int)b;
+      T.src_block = F.nbr_block;
+      T.pass = nout;
+      for (int a = 0; a < 3; ++a) {
+        T.lo[a] = side[a] == 0 ? -NG : (side[a] == 1 ? 0 : B.n[a]);
+        T.ext[a] = side[a] == 1 ? B.n[a] : NG;
+        T.shift[a] = F.shift[a];
+      }
+      const int an = F.face / 2, s = F.face % 2, sp = F.nbr_face % 2;
+      long long base = 0;
+      for (int a = 0; a < 3; ++a) {
+        const int ap = F.perm[a];
+        int sgn, off;
+        if (a == an) {
+          if (s == 0 && sp == 1) { sgn = 1; off = N.n[ap]; }
+          else if (s == 0 && sp == 0) { sgn = -1; off = -1; }
+          else if (s == 1 && sp == 0) { sgn = 1; off = -B.n[a]; }
+          else { sgn = -1; off = N.n[ap] + B.n[a] - 1; }
+        } else {
+          sgn = F.sign[a] > 0 ? 1 : -1;
+          off = F.sign[a] > 0 ? 0 : B.n[a] - 1;
+        }
+        T.sstride[a] = sgn * N.s[ap];
+        base += (long long)(off + NG) * N.s[ap];
+      }
+      T.sbase = base;
+      c->tasks[nout].push_back(T);
+    }
+  }
+}
+
+extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cfd_block_ptrs* ptrs, int nfaces,
+                                 const cfd_face* faces, const cfd_params* params, void* workspace, size_t workspace_bytes,
+                                 void* cuda_stream) {
+  if (!out || nblocks < 1 || !dims || !ptrs || !params || nfaces < 0 || (nfaces > 0 && !faces))
+    return fail_create(CFD_E_ARG, "cfd_create_blocks: null argument or nblocks < 1");
+  *out = nullptr;
+  if (!(params->gamma > 1.0) || !(params->weno_eps > 0.0) || !(params->weno_eps < 1e3))
+    return fail_create(CFD_E_ARG, "cfd_create_blocks: need gamma > 1 and 0 < weno_eps < 1e3");
+  if (params->viscous && (!(params->reynolds > 0.0) || !(params->prandtl > 0.0) || !(params->mach >= 0.0)))
+    return fail_create(CFD_E_ARG, "cfd_create_blocks: viscous run needs reynolds > 0, prandtl > 0, mach >= 0");
+  if (params->scheme != 0 && params->scheme != 1) return fail_create(CFD_E_ARG, "cfd_create_blocks: scheme must be 0 or 1");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+    return fail_create(CFD_E_CUDA, "cfd_create_blocks: no CUDA device (there is no CPU fallback)");
+
+  cfd_ctx* c = new cfd_ctx();
+  c->prm = *params;
+  c->pd.gamma = params->gamma;
+  c->pd.eps = params->weno_eps;
+  c->pd.viscous = params->viscous;
+  c->pd.mu = params->viscous ? params->mach / params->reynolds : 0.0;
+  c->pd.kappa = params->viscous ? c->pd.mu / (params->prandtl * (params->gamma - 1.0)) : 0.0;
+  for (int m = 0; m < 5; ++m) c->pd.q_inf[m] = params->q_inf[m];
+  c->stream = (cudaStream_t)cuda_stream;
+  c->blk.resize(nblocks);
+  for (int b = 0; b < nblocks; ++b) {
+    BlockDev& B = c->blk[b];
+    B.n[0] = dims[b].ni; B.n[1] = dims[b].nj; B.n[2] = dims[b].nk;
+    for (int a = 0; a < 3; ++a) {
+      if (B.n[a] < NG) { delete c; return fail_create(CFD_E_ARG, "cfd_create_blocks: interior size must be >= 6 on every axis"); }
+      B.m[a] = B.n[a] + 2 * NG;
+    }
+    B.M = (long long)B.m[0] * B.m[1] * B.m[2];
+    B.s[0] = 1; B.s[1] = B.m[0]; B.s[2] = (long long)B.m[0] * B.m[1];
+    B.q = ptrs[b].q; B.qn = ptrs[b].qn; B.r = ptrs[b].r; B.xyz = ptrs[b].xyz; B.khat = ptrs[b].khat; B.jac = ptrs[b].jac;
+    const void* pp[6] = {B.q, B.qn, B.r, B.xyz, B.khat, B.jac};
+    for (int t = 0; t < 6; ++t)
+      if (!pp[t] || ((uintptr_t)pp[t] & 15u)) { delete c; return fail_create(CFD_E_ARG, "cfd_create_blocks: null or misaligned (16 B) field pointer"); }
+    if (B.M > c->max_M) c->max_M = B.M;
+  }
+  // ---- faces ----
+  c->faces.assign(faces, faces + nfaces);
+  std::vector<int> seen((size_t)nblocks * 6, 0);
+  for (int t = 0; t < nfaces; ++t) {
+    const cfd_face& F = c->faces[t];
+    auto bad = [&](const char* m) { delete c; return fail_create(CFD_E_TOPOLOGY, std::string("cfd_create_blocks: face ") + std::to_string(t) + ": " + m); };
+    if (F.block < 0 || F.block >= nblocks || F.face < 0 || F.face > 5) return bad("bad block/face id");
+    if (seen[(size_t)F.block * 6 + F.face]++) return bad("described twice");
+    if (is_connect(F.type)) {
+      if (F.nbr_block < 0 || F.nbr_block >= nblocks || F.nbr_face < 0 || F.nbr_face > 5) return bad("bad neighbour");
+      int cnt[3] = {0, 0, 0};
+      for (int a = 0; a < 3; ++a) {
+        if (F.perm[a] < 0 || F.perm[a] > 2 || (F.sign[a] != 1 && F.sign[a] != -1)) return bad("bad perm/sign");
+        cnt[F.perm[a]]++;
+      }
+      if (cnt[0] != 1 || cnt[1] != 1 || cnt[2] != 1) return bad("perm is not a permutation");
+      const bool even = (F.perm[0] == 0 && F.perm[1] == 1) || (F.perm[0] == 1 && F.perm[1] == 2) || (F.perm[0] == 2 && F.perm[1] == 0);
+      if ((even ? 1 : -1) * F.sign[0] * F.sign[1] * F.sign[2] != 1) return bad("not a proper rotation");
+      const int an = F.face / 2;
+      if (F.perm[an] != F.nbr_face / 2) return bad("nbr_face axis != perm[normal axis]");
+      if (F.sign[an] != ((F.face % 2) != (F.nbr_face % 2) ? 1 : -1)) return bad("normal-axis sign inconsistent with the face pair");
+      for (int a = 0; a < 3; ++a)
+        if (a != an && c->blk[F.nbr_block].n[F.perm[a]] != c->blk[F.block].n[a]) return bad("interface extents do not match");
+    } else if (F.type == CFD_FACE_WALL_NOSLIP_ADIABATIC || F.type == CFD_FACE_FARFIELD_CHAR) {
+      BcTask T{F.block, F.face, F.type};
+      c->bcs.push_back(T);
+    } else {
+      return bad("unknown face type");
+    }
+  }
+  // ---- workspace ----
+  size_t need = cfd_workspace_bytes(nblocks, dims, params);
+  if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 15u)) {
+    delete c;
+    return fail_create(CFD_E_WORKSPACE, "cfd_create_blocks: workspace null, misaligned or smaller than cfd_workspace_bytes()");
+  }
+  c->ws = (double*)workspace;
+  c->ws_bytes = workspace_bytes;
+  plan_copies(c);
+  // ---- small device-side descriptor arrays (a few KB; the only allocations the library makes) ----
+  auto cuda_fail = [&](cudaError_t e, const char* what) {
+    std::string m = std::string("cfd_create_blocks: ") + what + ": " + cudaGetErrorString(e);
+    cfd_destroy(c);
+    return fail_create(CFD_E_CUDA, m);
+  };
+  cudaError_t e;
+  if ((e = cudaMalloc(&c->d_blocks, sizeof(BlockDev) * nblocks)) != cudaSuccess) return cuda_fail(e, "cudaMalloc blocks");
+  if ((e = cudaMemcpy(c->d_blocks, c->blk.data(), sizeof(BlockDev) * nblocks, cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy blocks");
+  for (int p = 1; p <= 3; ++p) {
+    if (c->tasks[p].empty()) continue;
+    if ((e = cudaMalloc(&c->d_tasks[p], sizeof(CopyTask) * c->tasks[p].size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc tasks");
+    if ((e = cudaMemcpy(c->d_tasks[p], c->tasks[p].data(), sizeof(CopyTask) * c->tasks[p].size(), cudaMemcpyHostToDevice)) != cudaSuccess)
+      return cuda_fail(e, "cudaMemcpy tasks");
+  }
+  if ((e = cudaMalloc(&c->d_flag, sizeof(int))) != cudaSuccess) return cuda_fail(e, "cudaMalloc flag");
+  if ((e = cudaMalloc(&c->d_res, sizeof(double) * 8)) != cudaSuccess) return cuda_fail(e, "cudaMalloc res");
+  *out = c;
+  return CFD_OK;
+}
+
+extern "C" int cfd_destroy(cfd_ctx* c) {
+  if (!c) return CFD_OK;
+  if (c->d_blocks) cudaFree(c->d_blocks);
+  for (int p = 1; p <= 3; ++p)
+    if (c->d_tasks[p]) cudaFree(c->d_tasks[p]);
+  if (c->d_flag) cudaFree(c->d_flag);
+  if (c->d_res) cudaFree(c->d_res);
+  delete c;
+  return CFD_OK;
+}
+
+extern "C" const char* cfd_last_error(const cfd_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+extern "C" long long cfd_launch_count(const cfd_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int cfd_compute_metrics(cfd_ctx* c) {
+  if (!c) return CFD_E_ARG;
+  int rc;
+  if ((rc = launch_fill_connect(c, 1)) != 0) return rc;
+  if ((rc = launch_bc_xyz(c)) != 0) return rc;
+  CUDA_TRY(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream));
+  if ((rc = launch_metrics(c)) != 0) return rc;
+  int flag = 0;
+  CUDA_TRY(c, cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (flag) { c->err = "cfd_compute_metrics: J <= 0 at an interior node"; return CFD_E_JACOBIAN; }
+  return CFD_OK;
+}
+
+extern "C" int cfd_rhs(cfd_ctx* c) {
+  if (!c) return CFD_E_ARG;
+  return launch_rhs(c);
+}
+
+extern "C" int cfd_rk_stage(cfd_ctx* c, int stage, double dt, double* res5) {
+  if (!c) return CFD_E_ARG;
+  if (stage < 1 || stage > 3) { c->err = "cfd_rk_stage: stage must be 1..3"; return CFD_E_STAGE; }
+  int rc = launch_rk(c, stage, dt);
+  if (rc != 0) return rc;
+  if (res5 && stage == 1) {
+    CUDA_TRY(c, cudaMemcpyAsync(res5, c->d_res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  }
+  return CFD_OK;
+}
+
+extern "C" int cfd_exchange_interfaces(cfd_ctx* c) {
+  if (!c) return CFD_E_ARG;
+  return launch_fill_connect(c, 0);
+}
+
+extern "C" int cfd_apply_bc(cfd_ctx* c) {
+  if (!c) return CFD_E_ARG;
+  return launch_bc_q(c);
+}
+
+extern "C" int cfd_stage(cfd_ctx* c, int stage, double dt, double* res5) {
+  int rc;
+  if ((rc = cfd_rhs(c)) != 0) return rc;
+  if ((rc = cfd_rk_stage(c, stage, dt, res5)) != 0) return rc;
+  if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
+  return cfd_apply_bc(c);
+}
+
+extern "C" int cfd_fp64_peak_probe(int iters, double* tflops) {
+  if (!tflops || iters < 1) return CFD_E_ARG;
+  return launch_fp64_probe(iters, tflops);
+}

@@ -1,0 +1,86 @@
+// Internal declarations of the sm_100a CUDA path (not part of the C ABI; see include/cfd.h).
+// Shares no code with oracle/.  P:L<n> = /root/reference/PAPER.md line n; U<k> = DESIGN.md reading k.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "cfd.h"
+
+#define NG CFD_NG
+
+// Device view of one block.  Strides in doubles: s[0] = 1, s[1] = m0, s[2] = m0*m1.
+struct BlockDev {
+  int n[3];
+  int m[3];
+  long long M;
+  long long s[3];
+  double *q, *qn, *r, *xyz, *khat, *jac;
+  // offset of interior node (0,0,0)
+  __host__ __device__ inline long long idx(int i, int j, int k) const {
+    return ((long long)(k + NG) * m[1] + (j + NG)) * m[0] + (i + NG);
+  }
+};
+
+struct ParamsDev {
+  double gamma, eps, mu, kappa;  // mu = Ma/Re (mu == 1, U9/U11), kappa = mu / (Pr (gamma-1))
+  double q_inf[5];
+  int viscous;
+};
+
+// One rectangular ghost region of one block, filled from a neighbour through an affine index map
+// (U15): src index along neighbour axis perm[a] = sgn[a] * (dst index along a) + off[a].
+struct CopyTask {
+  int dst_block, src_block;
+  int lo[3], ext[3];       // destination box: lo .. lo+ext-1 (interior-relative indices)
+  long long sstride[3];    // stride (in doubles) in the SOURCE array when the dst index a increases by one (signed)
+  long long sbase;         // source offset (doubles) of dst index (0,0,0) mapped
+  double shift[3];         // coordinate shift (xyz fill only)
+  int pass;                // 1 faces, 2 edges, 3 corners
+};
+
+struct BcTask {
+  int block, face, type;   // CFD_FACE_WALL_NOSLIP_ADIABATIC or CFD_FACE_FARFIELD_CHAR
+};
+
+struct cfd_ctx {
+  cfd_params prm;
+  ParamsDev pd;
+  std::vector<BlockDev> blk;
+  std::vector<cfd_face> faces;
+  std::vector<CopyTask> tasks[4];     // per pass 1..3
+  std::vector<BcTask> bcs;
+  CopyTask* d_tasks[4] = {nullptr, nullptr, nullptr, nullptr};
+  BlockDev* d_blocks = nullptr;
+  int* d_flag = nullptr;              // J <= 0 flag
+  double* d_res = nullptr;            // 5 residual sums
+  cudaStream_t stream = nullptr;
+  double* ws = nullptr;
+  size_t ws_bytes = 0;
+  long long max_M = 0;
+  long long launches = 0;
+  std::string err;
+};
+
+// ---- kernel launchers (each enqueues on ctx->stream and bumps ctx->launches) --------------------
+int launch_fill_connect(cfd_ctx* c, int field /*0 q, 1 xyz*/);
+int launch_bc_xyz(cfd_ctx* c);
+int launch_bc_q(cfd_ctx* c);
+int launch_metrics(cfd_ctx* c);
+int launch_rhs(cfd_ctx* c);
+int launch_rk(cfd_ctx* c, int stage, double dt);
+int launch_fp64_probe(int iters, double* tflops);
+
+size_t ws_partials_offset_doubles(long long max_M);
+int rk_max_partial_blocks();
+
+#define CUDA_TRY(ctx, expr)                                                      \
+  do {                                                                           \
+    cudaError_t _e = (expr);                                                     \
+    if (_e != cudaSuccess) {                                                     \
+      (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(_e);           \
+      return CFD_E_CUDA;                                                         \
+    }                                                                            \
+  } while (0)

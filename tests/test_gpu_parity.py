@@ -1,0 +1,309 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle element by
+element on the same seeded inputs.  Tolerances (BASELINE.json north_star): 1e-12 max relative error per
+RHS evaluation, normalised per equation by the magnitude of the summands S_m = max J * max_d |F^d_m|
+(SURVEY §8(d) "Parity normaliser"); 1e-10 on the state after 100 RK3 steps (smooth cases); integer /
+copy work (ghost fill) bit-exact."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+NG = 6
+RHS_TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2006_07964_b200 import binding
+
+    return binding
+
+
+def pair(po, B, case):
+    o = po.Oracle(case.dims, case.faces, case.params)
+    o.load_case(case)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    return o, g
+
+
+def flux_scale(o, b, gamma=1.4):
+    """S_m = max J * max over directions and points of |F^d_m(Q, khat^d)| on the interior (Eq. 4)."""
+    q = o.interior(b, "q")
+    kh = o.interior(b, "khat").reshape(3, 3, *q.shape[1:])
+    J = o.interior(b, "jac")[0]
+    u = q[1:4] / q[0]
+    p = (gamma - 1) * (q[4] - 0.5 * q[0] * (u ** 2).sum(0))
+    S = np.zeros(5)
+    for d in range(3):
+        th = (kh[d] * u).sum(0)
+        F = np.stack([q[0] * th, q[1] * th + kh[d, 0] * p, q[2] * th + kh[d, 1] * p, q[3] * th + kh[d, 2] * p, (q[4] + p) * th])
+        S = np.maximum(S, np.abs(F).max(axis=(1, 2, 3)))
+    return S * J.max()
+
+
+def assert_rhs_parity(o, g, case, tol=RHS_TOL):
+    o.rhs()
+    g.rhs()
+    worst = 0.0
+    for b in range(len(case.dims)):
+        S = flux_scale(o, b)
+        ro, rg = o.interior(b, "r"), g.to_numpy(b, "r")
+        assert np.isfinite(rg).all()
+        err = np.abs(rg - ro).max(axis=(1, 2, 3)) / S
+        worst = max(worst, err.max())
+        assert err.max() < tol, (case.name, b, err)
+    return worst
+
+
+# ------------------------------------------------------------------------------------------------
+# S1 metrics
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["c1", "wavy-ragged", "cylinder", "multiblock"])
+def test_metrics_parity(po, W, B, which):
+    case = {"c1": lambda: W.c1_vortex(32),
+            "wavy-ragged": lambda: ragged_case(W),
+            "cylinder": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0),
+            "multiblock": lambda: W.c4_multiblock(nb=12)}[which]()
+    o, g = pair(po, B, case)
+    for b in range(len(case.dims)):
+        xo, xg = o.field(b, "xyz"), g.to_numpy(b, "xyz", interior=False)
+        assert np.allclose(xg, xo, rtol=0, atol=1e-13 * np.abs(xo).max())
+        box = (slice(None),) + (slice(3, -3),) * 3
+        ko, kg = o.field(b, "khat")[box], g.to_numpy(b, "khat", interior=False)[box]
+        assert np.abs(kg - ko).max() < 1e-13 * np.abs(ko).max()
+        jo, jg = o.field(b, "jac")[box], g.to_numpy(b, "jac", interior=False)[box]
+        assert np.abs(jg / jo - 1).max() < 1e-12
+
+
+def ragged_case(W, viscous=1):
+    """Non-cubic block whose sizes are not multiples of any tile edge (62, 6, 32): several tiles + ragged tails."""
+    n = (71, 23, 15)
+    L = 2 * np.pi
+    X, Y, Z = W._uniform_nodes(n, (L, L, L))
+    modes = W.wavy_modes(11)
+    xyz = W.wavy_mapping(X, Y, Z, L, L / 23, modes, amp=0.25)
+    q0 = W.tgv_field(xyz, 0.4)
+    q0 = W.prim_to_cons(q0[0] * (1 + 0.1 * np.sin(xyz[1])), q0[1] / q0[0] + 0.2, q0[2] / q0[0], 0.1 * np.cos(xyz[0] + xyz[2]),
+                        (1 / 1.4) * (1 + 0.05 * np.cos(xyz[2])))
+    return W.Case("ragged", [n], [xyz], [q0], W.periodic_faces(0, (L, L, L)),
+                  W.default_params(viscous=viscous, mach=0.4, reynolds=300.0), dt=1e-3, steps=0)
+
+
+# ------------------------------------------------------------------------------------------------
+# S2 + S3: RHS parity, element by element
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["c1-euler", "tgv-ns", "ragged-ns", "ragged-euler", "multiblock-ns", "cylinder-ns", "tiny"])
+def test_rhs_parity(po, W, B, which):
+    case = {"c1-euler": lambda: W.c1_vortex(32),
+            "tgv-ns": lambda: W.tgv_sine_box(24, viscous=1, mach=0.4),
+            "ragged-ns": lambda: ragged_case(W, 1),
+            "ragged-euler": lambda: ragged_case(W, 0),
+            "multiblock-ns": lambda: W.c4_multiblock(nb=12, mach=0.3),
+            "cylinder-ns": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0, noise=1e-2),
+            "tiny": lambda: W.tgv_sine_box(6, viscous=1, mach=0.3)}[which]()  # minimum block size (degenerate tiles)
+    o, g = pair(po, B, case)
+    assert_rhs_parity(o, g, case)
+
+
+def test_rhs_parity_strong_gradients(po, W, B):
+    """Non-smooth data (the WENO weights far from the linear ones): seeded random +-20 % perturbation per node."""
+    case = W.c1_vortex(24)
+    rng = np.random.default_rng(99)
+    q = case.q0[0]
+    rho = q[0] * (1 + 0.2 * rng.uniform(-1, 1, q[0].shape))
+    p = (1 / 1.4) * (1 + 0.2 * rng.uniform(-1, 1, q[0].shape))
+    case.q0[0] = W.prim_to_cons(rho, q[1] / q[0], q[2] / q[0] + 0.3 * rng.uniform(-1, 1, q[0].shape), q[3] / q[0], p)
+    o, g = pair(po, B, case)
+    assert_rhs_parity(o, g, case)
+
+
+def test_free_stream_on_gpu(po, W, B):
+    """Config 2 (reduced to 32^3): uniform flow on the seeded wavy grid stays at round-off on the GPU itself."""
+    case = W.c2_freestream(32, viscous=1)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    g.rhs()
+    r = g.to_numpy(0, "r")
+    J = g.to_numpy(0, "jac")
+    kh = g.to_numpy(0, "khat")
+    assert np.abs(r).max() < 1e-12 * J.max() * np.abs(kh).max() * 3
+    q0 = g.to_numpy(0, "q").copy()
+    for _ in range(100):
+        g.step(case.dt)
+    assert np.abs(g.to_numpy(0, "q") - q0).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# S6 / S5: ghost fill (bit-exact) and boundary conditions
+# ------------------------------------------------------------------------------------------------
+def test_exchange_is_bit_exact_with_signed_permutations(po, W, B):
+    case = W.c4_multiblock(nb=10, mach=0.3)
+    assert any(f["perm"] != [0, 1, 2] for f in case.faces)
+    o, g = pair(po, B, case)
+    for b in range(8):
+        assert np.array_equal(g.to_numpy(b, "q", interior=False), o.field(b, "q"))
+    # scramble the ghosts on the GPU, exchange again
+    for b in range(8):
+        f = g.fields[b]["q"]
+        keep = f[:, NG:-NG, NG:-NG, NG:-NG].clone()
+        f.fill_(float("nan"))
+        f[:, NG:-NG, NG:-NG, NG:-NG] = keep
+    g.exchange_interfaces()
+    for b in range(8):
+        assert np.array_equal(g.to_numpy(b, "q", interior=False), o.field(b, "q"))
+
+
+def test_bc_parity_cylinder(po, W, B):
+    case = W.c5_cylinder(ni=48, nj=20, nk=8, ratio=1.2, r_out=8.0, noise=1e-2)
+    o, g = pair(po, B, case)
+    qo, qg = o.field(0, "q"), g.to_numpy(0, "q", interior=False)
+    t = slice(3, -3)  # tangential range the BCs define
+    assert np.allclose(qg[:, t, :, t], qo[:, t, :, t], rtol=1e-13, atol=1e-15)
+    assert np.all(qg[1:4, t, NG, t] == 0.0)
+
+
+# ------------------------------------------------------------------------------------------------
+# S4 and whole steps
+# ------------------------------------------------------------------------------------------------
+def test_rk_stage_and_residual(po, W, B):
+    case = ragged_case(W, 1)
+    o, g = pair(po, B, case)
+    o.rhs()
+    g.rhs()
+    dt = 1e-3
+    for s in (1, 2, 3):
+        ro = o.rk_stage(s, dt, want_res=True)
+        rg = g.rk_stage(s, dt, want_res=True)
+        if s == 1:
+            assert np.allclose(rg, ro, rtol=1e-12)
+        assert np.abs(g.to_numpy(0, "q") - o.interior(0, "q")).max() < 1e-13
+    assert np.abs(g.to_numpy(0, "qn") - o.interior(0, "qn")).max() < 1e-13
+    # deterministic reduction: bit-identical on repetition
+    g.rhs()
+    a = g.rk_stage(1, 0.0, want_res=True)
+    g.rhs()
+    b = g.rk_stage(1, 0.0, want_res=True)
+    assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("which", ["c1", "multiblock", "cylinder"])
+def test_state_parity_after_steps(po, W, B, which):
+    case, nsteps = {"c1": lambda: (W.c1_vortex(32), 10),  # config 1 as specified: 10 RK3 steps at CFL 0.5
+                    "multiblock": lambda: (W.c4_multiblock(nb=12, mach=0.3), 6),
+                    "cylinder": lambda: (W.c5_cylinder(ni=48, nj=20, nk=8, ratio=1.2, r_out=8.0, noise=1e-3), 6)}[which]()
+    o, g = pair(po, B, case)
+    dt = o.cfl_dt(0.5)
+    for _ in range(nsteps):
+        ro = o.step(dt)
+        rg = g.step(dt, want_res=True)
+    assert np.allclose(rg, ro, rtol=1e-9)
+    for b in range(len(case.dims)):
+        qo, qg = o.interior(b, "q"), g.to_numpy(b, "q")
+        assert np.abs(qg - qo).max() < 1e-11 * np.abs(qo).max()
+    if which == "c1":
+        exact = W.vortex_field(case.xyz[0], t=nsteps * dt)
+        assert np.abs(g.to_numpy(0, "q") - exact).max() < 0.05
+
+
+def test_state_parity_after_100_steps_smooth(po, W, B):
+    """north_star: 1e-10 after 100 RK3 steps on smooth cases (TGV, viscous, wavy grid; reduced to 24^3)."""
+    case = W.c3_tgv(n=24, viscous=1, mach=0.1)
+    o, g = pair(po, B, case)
+    dt = o.cfl_dt(0.5)
+    for _ in range(100):
+        o.step(dt)
+        g.step(dt)
+    qo, qg = o.interior(0, "q"), g.to_numpy(0, "q")
+    assert np.abs(qg - qo).max() < 1e-10 * np.abs(qo).max()
+
+
+# ------------------------------------------------------------------------------------------------
+# Full-size configs in the launch configuration bench.py times: sampled sub-boxes.  The GPU's own q,
+# khat, jac (with ghosts) are cut out around sample points and handed to the oracle as a face-less block;
+# the oracle's RHS on the sub-box interior must match the GPU's RHS there.
+# ------------------------------------------------------------------------------------------------
+def subbox_check(po, g, case, b, lo, ext, S):
+    sl = tuple(slice(lo[a], lo[a] + ext[a] + 2 * NG) for a in (2, 1, 0))  # array coordinates (ghost offset included)
+    o = po.Oracle([tuple(ext)], [], case.params)
+    for name in ("q", "khat", "jac"):
+        o.field(0, name)[...] = g.fields[b][name][(slice(None),) + sl].cpu().numpy()
+    o.rhs()
+    isl = tuple(slice(lo[a] + NG, lo[a] + NG + ext[a]) for a in (2, 1, 0))
+    rg = g.fields[b]["r"][(slice(None),) + isl].cpu().numpy()
+    err = np.abs(rg - o.interior(0, "r")).max(axis=(1, 2, 3)) / S
+    assert err.max() < RHS_TOL, (case.name, b, lo, err)
+
+
+def sample_boxes(n, rng, ext=(14, 10, 8), count=5):
+    boxes = [(0, 0, 0), tuple(n[a] - ext[a] for a in range(3))]  # the two extreme corners
+    for _ in range(count):
+        boxes.append(tuple(int(rng.integers(0, n[a] - ext[a] + 1)) for a in range(3)))
+    return boxes, ext
+
+
+@pytest.mark.parametrize("which", ["C2-64", "C3-128", "C4-8x96", "C5-cylinder", "sweep-256"])
+def test_full_size_sampled_parity(po, W, B, which):
+    import torch
+
+    case = {"C2-64": lambda: W.c2_freestream(64), "C3-128": lambda: W.c3_tgv(128), "C4-8x96": lambda: W.c4_multiblock(96),
+            "C5-cylinder": lambda: W.c5_cylinder(), "sweep-256": lambda: W.sweep_block(256)}[which]()
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    g.step(case.dt)  # one full step first so that the sampled state is not the analytic initial field
+    g.rhs()
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(1234)
+    for b in range(len(case.dims)):
+        if b not in (0, len(case.dims) - 1):
+            continue
+        n = case.dims[b]
+        q = g.interior(b, "q")
+        assert torch.isfinite(q).all()
+        # flux scale from the GPU state (tolerance normaliser only)
+        u = (q[1:4] / q[0])
+        p = 0.4 * (q[4] - 0.5 * q[0] * (u ** 2).sum(0))
+        kh = g.interior(b, "khat").reshape(3, 3, *q.shape[1:])
+        J = g.interior(b, "jac")[0]
+        S = np.zeros(5)
+        for d in range(3):
+            th = (kh[d] * u).sum(0)
+            F = [q[0] * th, q[1] * th + kh[d, 0] * p, q[2] * th + kh[d, 1] * p, q[3] * th + kh[d, 2] * p, (q[4] + p) * th]
+            S = np.maximum(S, np.array([float(f.abs().max()) for f in F]))
+        S = S * float(J.max())
+        boxes, ext = sample_boxes(n, rng)
+        for lo in boxes:
+            subbox_check(po, g, case, b, lo, ext, S)
+
+
+# ------------------------------------------------------------------------------------------------
+# error behaviour through the ABI
+# ------------------------------------------------------------------------------------------------
+def test_error_codes(W, B):
+    case = W.c1_vortex(8)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    with pytest.raises(B.CfdError) as e:
+        g.rk_stage(4, 0.1)
+    assert e.value.code == -4
+    bad = [dict(f) for f in case.faces]
+    bad[0]["sign"] = [-1, 1, 1]
+    with pytest.raises(B.CfdError) as e:
+        B.Context(case.dims, bad, case.params)
+    assert e.value.code == -2
+    with pytest.raises(B.CfdError) as e:
+        B.Context([(4, 8, 8)], [], case.params)
+    assert e.value.code == -1
+    # left-handed grid -> J < 0
+    flipped = W.c1_vortex(8)
+    flipped.xyz[0] = flipped.xyz[0][:, :, :, ::-1].copy()
+    for f in flipped.faces:
+        if f["face"] in (0, 1):
+            f["shift"] = [-f["shift"][0], 0.0, 0.0]
+    g2 = B.Context(flipped.dims, flipped.faces, flipped.params)
+    with pytest.raises(B.CfdError) as e:
+        g2.load_case(flipped)
+    assert e.value.code == -3
