@@ -1,0 +1,424 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the fp64 curvilinear RHS + RK-stage hot path (arxiv 2006.07964) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+A "step" is one TVD-RK3 time step = three passes of the whole hot path (S2+S3 cfd_rhs, S4 cfd_rk_stage,
+S6 cfd_exchange_interfaces, S5 cfd_apply_bc; Fig. 2) over every block of the workload.
+Metric (BASELINE.json): fp64 grid-point updates per second per RK stage, in Gpts/s
+    value = (interior points of all blocks) x 3 stages x K / elapsed            (inputs resident in HBM)
+    e2e   = the same through cfd_step_host with HOST buffers (H2D + D2H inside the timed region).
+Prints ONE JSON line on rank 0.  The path does not shard ("replicas only"): with --gpus N
+every rank runs the same workload on its own GPU, no data-path collective; scaling = "weak".
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on the host cores instead: this tier
+has no reference implementation to install, the oracle IS the reference arm.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 grid-point updates/sec per RK stage (Gpts/s); % of HBM/FP64 roofline"
+UNIT = "Gpts/s"
+
+# Algorithmic flops per interior point (add, sub, mul, div, sqrt = 1 each; FMA = 2), the exact count of the
+# oracle's per-point routines run with a counting scalar (oracle/flopcount.cpp; tests/test_flopcount.py
+# checks these constants against that program).  DESIGN.md section 7.
+FLOPS_PER_POINT = {"inviscid_dir": 1381, "viscous": 478, "rk": 25, "ns_stage": 4671, "euler_stage": 4193}
+# Algorithmic bytes per interior point per stage: read Q 5 + khat,J 10 + Q^n 5, write Q 5 doubles.
+BYTES_PER_POINT_STAGE = 200
+# FP64 ALU peak derived from unit counts and clocks: 148 SMs x 4 sub-partitions x 16 FP64
+# FMA lanes x 2 flop x 1.965 GHz (clocks.max.sm).  The live DFMA probe is reported next to it.
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+HBM_FALLBACK_GBS = 6650.0
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/), keyed by (workload, kernel class); None until captured.
+NCU_TRAFFIC_BYTES = {}
+
+WORKLOADS = {
+    "c1": "C1 32^3 isentropic vortex, Euler, periodic, warped box",
+    "c2": "C2 64^3 free stream on seeded wavy grid, Navier-Stokes, periodic",
+    "c3": "C3 128^3 Taylor-Green vortex, Navier-Stokes Re=1600 Ma=0.1, seeded wavy grid, periodic",
+    "c4": "C4 8 x 96^3 point-matched blocks with seeded signed index permutations, Navier-Stokes TGV",
+    "c5": "C5 cylinder O-grid 1024x256x128, Navier-Stokes Re=3900 Ma=0.2, wall + far field",
+    "sweep256": "sweep 256^3 (C3 mapping and field), Navier-Stokes, periodic",
+    "sweep384": "sweep 384^3 (C3 mapping and field), Navier-Stokes, periodic",
+    "sweep512": "sweep 512^3 (C3 mapping and field), Navier-Stokes, periodic",
+    "sweep256-euler": "sweep 256^3 (C3 mapping and field), Euler, periodic",
+}
+
+
+def make_case(name):
+    from paper_2006_07964_b200 import workloads as W
+
+    if name == "c1":
+        return W.c1_vortex(32)
+    if name == "c2":
+        return W.c2_freestream(64)
+    if name == "c3":
+        return W.c3_tgv(128)
+    if name == "c4":
+        return W.c4_multiblock(96)
+    if name == "c5":
+        return W.c5_cylinder()
+    if name.startswith("sweep"):
+        n = int(name[5:8])
+        return W.sweep_block(n=n, viscous=0 if name.endswith("euler") else 1)
+    raise SystemExit(f"unknown workload {name}; choose from {sorted(WORKLOADS)}")
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# CPU oracle arm (test infrastructure, timed as it stands: cpu_baseline and --impl reference only)
+# ---------------------------------------------------------------------------------------------------------
+def sample_case(name):
+    """A BOUNDED sample of the workload for the CPU oracle: the same seeded recipe at a size that costs about
+    10-30 s of CPU work per RK3 step on one core (oracle: ~3.6 us per point-stage single-threaded)."""
+    from paper_2006_07964_b200 import workloads as W
+
+    if name in ("c1", "c2"):
+        return make_case(name), f"the full workload {name}"
+    if name == "c3":
+        return W.c3_tgv(96), "C3 recipe (same seed, mapping, field) generated at 96^3 instead of 128^3"
+    if name == "c4":
+        return W.c4_multiblock(48), "C4 recipe (same seed, permutations, field) with 8 blocks of 48^3 instead of 96^3"
+    if name == "c5":
+        return W.c5_cylinder(ni=256, nj=64, nk=32), "C5 recipe (same stretching ratio, BCs, noise seed) at 256x64x32"
+    n = 96
+    return (W.sweep_block(n=n, viscous=0 if name.endswith("euler") else 1),
+            f"sweep recipe (C3 seed, mapping, field) generated at {n}^3")
+
+
+def time_oracle(name, steps, warmup, threads=None):
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import pyoracle as po
+
+    case, what = sample_case(name)
+    o = po.Oracle(case.dims, case.faces, case.params, threads=threads)
+    o.load_case(case)
+    for _ in range(warmup):
+        o.step(case.dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(case.dt)
+    el = time.perf_counter() - t0
+    pts = case.npoints
+    return dict(value=pts * 3 * steps / el / 1e9, seconds=el, cores=int(o.threads), points=pts, steps=steps,
+                sample=f"{what}; {steps} RK3 step(s) = {pts * 3 * steps} point-stages", viscous=int(case.params["viscous"]))
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores (all OpenMP threads), same metric/unit/config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    r = time_oracle(args.workload, max(1, args.steps), min(args.warmup, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": r["seconds"] / max(1, args.steps) * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.workload], "name": args.workload, "stages_per_step": 3,
+                   "viscous": r["viscous"], "sample": r["sample"]},
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# GPU arm
+# ---------------------------------------------------------------------------------------------------------
+def dominant_roofline(prof, case, n_steps, hbm_gbs, hbm_src, dfma_probe_tflops, workload):
+    """Roofline of the dominant kernel class: algorithmic flops per launch / average launch duration (CUDA
+    events around every launch inside the timed region, cfd_profile_*), against the FP64 ALU peak; the HBM
+    term of the same kernel is reported beside it.  DESIGN.md section 7."""
+    if not prof:
+        return None
+    total_ms = sum(ms for ms, _ in prof.values())
+    name, (ms, launches) = max(prof.items(), key=lambda kv: kv[1][0])
+    pts = case.npoints
+    visc = int(case.params["viscous"])
+    nblocks = len(case.dims)
+    pts_per_launch = pts / nblocks
+    if name.startswith("inviscid") or name.startswith("sweep"):
+        flop_pt = FLOPS_PER_POINT["inviscid_dir"]
+    elif name.startswith("rhs_fused"):
+        flop_pt = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"] - FLOPS_PER_POINT["rk"]
+    elif name.startswith("visc"):
+        flop_pt = FLOPS_PER_POINT["viscous"]
+    else:
+        flop_pt = FLOPS_PER_POINT["rk"]
+    avg_s = ms * 1e-3 / launches
+    achieved = flop_pt * pts_per_launch / avg_s / 1e12
+    traffic = NCU_TRAFFIC_BYTES.get((workload, name))
+    return {
+        "bound": "alu", "kernel": name, "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+        "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": traffic,
+        "peak_source": "nominal FP64 FMA peak 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md s7); live DFMA probe beside it",
+        "peak_dfma_probe_tflops": dfma_probe_tflops,
+        "flop_per_point": flop_pt, "points_per_launch": pts_per_launch, "avg_launch_ms": avg_s * 1e3,
+        "launches_timed": launches, "share_of_step": ms / total_ms if total_ms > 0 else None,
+        "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
+        "kernel_ms_per_step": {k: v[0] / n_steps for k, v in prof.items()},
+    }
+
+
+def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True):
+    import torch
+
+    from paper_2006_07964_b200 import binding as B
+
+    case = make_case(name)
+    ctx = B.Context(case.dims, case.faces, case.params, device=device)
+    ctx.load_case(case)
+    pts = case.npoints
+    dt = case.dt
+    torch.cuda.synchronize(device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    for _ in range(warmup):
+        ctx.step(dt)
+    barrier()
+    l0 = ctx.launch_count
+    if profile:
+        ctx.profile_enable(True)
+    didx = torch.device(device).index or 0
+    try:
+        gpu_id = "GPU-" + str(torch.cuda.get_device_properties(didx).uuid)  # robust to CUDA_VISIBLE_DEVICES remapping
+    except Exception:
+        gpu_id = str(didx)
+    sampler = ClockSampler(gpu_id)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(ctx.stream)
+    for _ in range(steps):
+        ctx.step(dt)
+    e1.record(ctx.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    prof = ctx.profile_read() if profile else {}
+    if profile:
+        ctx.profile_enable(False)
+    launches = ctx.launch_count - l0
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    out = dict(case=case, ms=ms, pts=pts, launches=launches, prof=prof, clocks=clocks, finite=None)
+
+    # sanity: the state must still be finite (a blown-up run would time garbage)
+    out["finite"] = bool(all(torch.isfinite(ctx.interior(b, "q")).all().item() for b in range(len(case.dims))))
+
+    if e2e:
+        qh = [torch.empty((5, nk, nj, ni), dtype=torch.float64).pin_memory() for (ni, nj, nk) in case.dims]
+        for b in range(len(case.dims)):
+            qh[b].copy_(ctx.interior(b, "q"))
+        torch.cuda.synchronize(device)
+        ctx.step_host(qh, qh, dt)  # warm-up
+        barrier()
+        e0.record(ctx.stream)
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            ctx.step_host(qh, qh, dt)
+        e1.record(ctx.stream)
+        barrier()
+        wall = (time.perf_counter() - t0) * 1e3
+        ems = max(e0.elapsed_time(e1), 0.0)
+        if dist is not None:
+            t = torch.tensor([ems], dtype=torch.float64, device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        nbytes = sum(q.numel() * 8 for q in qh)
+        out["e2e"] = dict(ms=ems, wall_ms=wall, h2d=nbytes, d2h=nbytes,
+                          finite=bool(all(torch.isfinite(q).all().item() for q in qh)))
+        del qh
+    ctx.close()
+    del ctx
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback (use --impl reference for the oracle)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    device = f"cuda:{local}"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist_mod.init_process_group(backend="nccl", device_id=torch.device(device))
+        dist = dist_mod
+
+    from paper_2006_07964_b200 import binding as B
+
+    hbm_gbs, hbm_src = load_peaks()
+    probe = B.device_peak_probe(2048)
+    main = measure_gpu(args.workload, args.steps, args.warmup, device, dist=dist, e2e=True, profile=True)
+    case, pts = main["case"], main["pts"]
+    visc = int(case.params["viscous"])
+    n_stage = 3 * args.steps
+    value = world * pts * n_stage / (main["ms"] * 1e-3) / 1e9
+    e2e = main["e2e"]
+    e2e_value = world * pts * n_stage / (e2e["ms"] * 1e-3) / 1e9
+    flop_stage = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"]
+    per_gpu = value / world
+    t_alu = flop_stage / (FP64_PEAK_NOMINAL_TFLOPS * 1e12)
+    t_hbm = BYTES_PER_POINT_STAGE / (hbm_gbs * 1e9)
+    roof_gpts = 1.0 / max(t_alu, t_hbm) / 1e9
+
+    also = {}
+    if world == 1 and not args.no_also:
+        for w in args.also.split(","):
+            w = w.strip()
+            if not w or w == args.workload:
+                continue
+            try:
+                r = measure_gpu(w, max(2, min(args.steps, 3)), 3, device, dist=None, e2e=False, profile=False)
+                v = r["pts"] * 3 * max(2, min(args.steps, 3)) / (r["ms"] * 1e-3) / 1e9
+                fl = FLOPS_PER_POINT["ns_stage" if int(r["case"].params["viscous"]) else "euler_stage"]
+                also[w] = {"value": v, "unit": UNIT, "points": r["pts"], "finite": r["finite"],
+                           "roofline_frac_stage": v * 1e9 * max(fl / (FP64_PEAK_NOMINAL_TFLOPS * 1e12), t_hbm)}
+            except Exception as ex:  # a side measurement must never lose the main line
+                also[w] = {"error": f"{type(ex).__name__}: {ex}"[:200]}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        r = time_oracle(args.workload, 1, 0)
+        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+               "seconds": r["seconds"]}
+        cpu["gpu_over_cpu"] = value / r["value"]
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": main["ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.workload], "name": args.workload, "blocks": len(case.dims),
+                       "points": pts, "stages_per_step": 3, "viscous": visc, "dt": case.dt,
+                       "l2_policy": "inputs larger than L2 (state+metrics per stage >> 126 MB)" if pts * 200 > 2.5e8
+                       else "inputs SMALLER than L2 (small parity config; not a bandwidth claim)",
+                       "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+            "state_finite": main["finite"],
+            "stage_roofline": {"roofline_gpts": roof_gpts, "frac": per_gpu / roof_gpts, "flop_per_point_stage": flop_stage,
+                               "bytes_per_point_stage": BYTES_PER_POINT_STAGE, "alu_peak_tflops": FP64_PEAK_NOMINAL_TFLOPS,
+                               "hbm_peak_gbs": hbm_gbs, "achieved_tflops": per_gpu * 1e9 * flop_stage / 1e12,
+                               "achieved_alg_gbs": per_gpu * BYTES_PER_POINT_STAGE},
+            "roofline": dominant_roofline(main["prof"], case, args.steps, hbm_gbs, hbm_src, probe, args.workload),
+            "cpu_baseline": cpu,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
+                    "ms_per_step": e2e["ms"] / args.steps, "finite": e2e["finite"]},
+            "gpu_launches": main["launches"],
+            "clocks": main["clocks"],
+            "other_workloads": also,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="sweep256", choices=sorted(WORKLOADS))
+    ap.add_argument("--also", default="c3,c4,c5", help="comma list of extra workloads measured briefly (N=1 only)")
+    ap.add_argument("--no-also", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

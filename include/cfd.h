@@ -125,6 +125,23 @@ int cfd_apply_bc(cfd_ctx*);
 /* Convenience: the four calls above for one stage, in Fig. 2's order, on the context's stream. */
 int cfd_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
 
+/* End-to-end entry with HOST buffers (bench.py's e2e leg): for every block b, copies the interior state
+ * q_in_host[b] (layout [5][nk][nj][ni], fp64, i fastest, no ghost layers; pinned memory recommended)
+ * into the device q, fills ghosts (S6, S5), runs one TVD-RK3 step (three cfd_stage calls, Eq. 20,
+ * P:L173–180), copies the interior of q back into q_out_host[b] (same layout; may alias q_in_host[b])
+ * and synchronises the stream.  res5_host_or_null as in cfd_rk_stage.  Returns host values. */
+int cfd_step_host(cfd_ctx*, const double* const* q_in_host, double* const* q_out_host, double dt,
+                  double* res5_host_or_null);
+
+/* Per-kernel device timing (bench.py's roofline leg).  While enabled, every kernel launch of the hot
+ * path is bracketed by CUDA events on the context's stream.  cfd_profile_read synchronises the stream,
+ * writes, for each kernel class id < CFD_PROF_NCLASS, the summed device time in ms and the number of
+ * launches since the last read, and resets the counters.  cfd_profile_name(id) is a static string. */
+#define CFD_PROF_NCLASS 12
+int cfd_profile_enable(cfd_ctx*, int on);
+int cfd_profile_read(cfd_ctx*, double ms[CFD_PROF_NCLASS], long long launches[CFD_PROF_NCLASS]);
+const char* cfd_profile_name(int id);
+
 /* Frees the context (never the caller's buffers). */
 int cfd_destroy(cfd_ctx*);
 

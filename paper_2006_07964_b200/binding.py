@@ -18,8 +18,10 @@ LIB_PATH = os.path.join(HERE, "libcfd_b200.so")
 ABI_SYMBOLS = (
     "cfd_workspace_bytes", "cfd_create_blocks", "cfd_compute_metrics", "cfd_rhs", "cfd_rk_stage",
     "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
-    "cfd_launch_count", "cfd_fp64_peak_probe",
+    "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
+    "cfd_profile_name",
 )
+PROF_NCLASS = 12
 
 
 class CfdError(RuntimeError):
@@ -67,6 +69,14 @@ def _load():
     L.cfd_last_error.argtypes = [C.c_void_p]
     L.cfd_launch_count.restype = C.c_longlong
     L.cfd_launch_count.argtypes = [C.c_void_p]
+    L.cfd_step_host.restype = C.c_int
+    L.cfd_step_host.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_double, C.POINTER(C.c_double)]
+    L.cfd_profile_enable.restype = C.c_int
+    L.cfd_profile_enable.argtypes = [C.c_void_p, C.c_int]
+    L.cfd_profile_read.restype = C.c_int
+    L.cfd_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.cfd_profile_name.restype = C.c_char_p
+    L.cfd_profile_name.argtypes = [C.c_int]
     L.cfd_fp64_peak_probe.restype = C.c_int
     L.cfd_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
     return L
@@ -195,6 +205,39 @@ class Context:
             if s == 1:
                 res = r
         return res
+
+    def step_host(self, q_in, q_out, dt, want_res=False):
+        """cfd_step_host: q_in / q_out are lists (one per block) of HOST fp64 tensors or numpy arrays of shape
+        (5, nk, nj, ni), C-contiguous (pinned torch tensors recommended); returns res5 or None."""
+        nb = len(self.dims)
+        pin = (C.c_void_p * nb)(*[self._host_ptr(a, b) for b, a in enumerate(q_in)])
+        pout = (C.c_void_p * nb)(*[self._host_ptr(a, b) for b, a in enumerate(q_out)])
+        res = (C.c_double * 5)()
+        self._chk(lib.cfd_step_host(self.h, pin, pout, float(dt), res if want_res else None))
+        return np.array(res[:]) if want_res else None
+
+    def _host_ptr(self, a, b):
+        ni, nj, nk = self.dims[b]
+        if isinstance(a, np.ndarray):
+            ok = a.dtype == np.float64 and a.flags["C_CONTIGUOUS"] and a.shape == (5, nk, nj, ni)
+            ptr = a.ctypes.data
+        else:
+            ok = (a.dtype == self.torch.float64 and a.is_contiguous() and tuple(a.shape) == (5, nk, nj, ni)
+                  and a.device.type == "cpu")
+            ptr = a.data_ptr()
+        if not ok:
+            raise CfdError(-1, f"step_host: block {b} needs a C-contiguous host fp64 array of shape (5,{nk},{nj},{ni})")
+        return ptr
+
+    def profile_enable(self, on=True):
+        self._chk(lib.cfd_profile_enable(self.h, 1 if on else 0))
+
+    def profile_read(self):
+        """{kernel class: (summed device ms, launches)} since the last read (synchronises)."""
+        ms = (C.c_double * PROF_NCLASS)()
+        n = (C.c_longlong * PROF_NCLASS)()
+        self._chk(lib.cfd_profile_read(self.h, ms, n))
+        return {lib.cfd_profile_name(i).decode(): (ms[i], int(n[i])) for i in range(PROF_NCLASS) if n[i]}
 
     @property
     def launch_count(self):

@@ -186,6 +186,7 @@ extern "C" int cfd_destroy(cfd_ctx* c) {
     if (c->d_tasks[p]) cudaFree(c->d_tasks[p]);
   if (c->d_flag) cudaFree(c->d_flag);
   if (c->d_res) cudaFree(c->d_res);
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;
   return CFD_OK;
 }
@@ -240,6 +241,71 @@ extern "C" int cfd_stage(cfd_ctx* c, int stage, double dt, double* res5) {
   if ((rc = cfd_rk_stage(c, stage, dt, res5)) != 0) return rc;
   if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
   return cfd_apply_bc(c);
+}
+
+extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const* qout, double dt, double* res5) {
+  if (!c || !qin || !qout) return CFD_E_ARG;
+  auto copy3d = [&](const BlockDev& B, double* dev, double* host, bool to_dev) {
+    cudaMemcpy3DParms p;
+    memset(&p, 0, sizeof(p));
+    cudaPitchedPtr d = make_cudaPitchedPtr(dev, (size_t)B.m[0] * 8, (size_t)B.m[0] * 8, (size_t)B.m[1]);
+    cudaPitchedPtr h = make_cudaPitchedPtr(host, (size_t)B.n[0] * 8, (size_t)B.n[0] * 8, (size_t)B.n[1]);
+    const cudaPos dpos = make_cudaPos((size_t)NG * 8, NG, NG), hpos = make_cudaPos(0, 0, 0);
+    p.srcPtr = to_dev ? h : d; p.srcPos = to_dev ? hpos : dpos;
+    p.dstPtr = to_dev ? d : h; p.dstPos = to_dev ? dpos : hpos;
+    p.extent = make_cudaExtent((size_t)B.n[0] * 8, (size_t)B.n[1], (size_t)B.n[2]);
+    p.kind = to_dev ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
+    return cudaMemcpy3DAsync(&p, c->stream);
+  };
+  for (size_t b = 0; b < c->blk.size(); ++b) {
+    const BlockDev& B = c->blk[b];
+    if (!qin[b] || !qout[b]) { c->err = "cfd_step_host: null host pointer"; return CFD_E_ARG; }
+    const size_t N = (size_t)B.n[0] * B.n[1] * B.n[2];
+    ProfScope ps(c, PK_COPY);
+    for (int m = 0; m < 5; ++m) CUDA_TRY(c, copy3d(B, B.q + (size_t)m * B.M, const_cast<double*>(qin[b]) + m * N, true));
+  }
+  int rc;
+  if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
+  if ((rc = cfd_apply_bc(c)) != 0) return rc;
+  for (int s = 1; s <= 3; ++s)
+    if ((rc = cfd_stage(c, s, dt, nullptr)) != 0) return rc;
+  for (size_t b = 0; b < c->blk.size(); ++b) {
+    const BlockDev& B = c->blk[b];
+    const size_t N = (size_t)B.n[0] * B.n[1] * B.n[2];
+    ProfScope ps(c, PK_COPY);
+    for (int m = 0; m < 5; ++m) CUDA_TRY(c, copy3d(B, B.q + (size_t)m * B.M, qout[b] + m * N, false));
+  }
+  if (res5) CUDA_TRY(c, cudaMemcpyAsync(res5, c->d_res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return CFD_OK;
+}
+
+static const char* k_prof_names[CFD_PROF_NCLASS] = {"inviscid_xi", "inviscid_eta", "inviscid_zeta", "visc_flux", "visc_div", "rk_stage",
+                                                    "residual_final", "ghost_fill", "phys_bc", "metrics", "host_copy", "other"};
+
+extern "C" const char* cfd_profile_name(int id) { return (id >= 0 && id < CFD_PROF_NCLASS) ? k_prof_names[id] : ""; }
+
+extern "C" int cfd_profile_enable(cfd_ctx* c, int on) {
+  if (!c) return CFD_E_ARG;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  c->prof_on = on != 0;
+  c->prof_used = 0;
+  return CFD_OK;
+}
+
+extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
+  if (!c || !ms || !launches) return CFD_E_ARG;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < CFD_PROF_NCLASS; ++i) { ms[i] = 0.0; launches[i] = 0; }
+  for (size_t t = 0; t + 1 < c->prof_used; t += 2) {
+    float e = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&e, c->prof_ev[t], c->prof_ev[t + 1]));
+    const int id = c->prof_id[t / 2];
+    ms[id] += e;
+    launches[id] += 1;
+  }
+  c->prof_used = 0;
+  return CFD_OK;
 }
 
 extern "C" int cfd_fp64_peak_probe(int iters, double* tflops) {

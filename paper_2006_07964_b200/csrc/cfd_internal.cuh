@@ -62,6 +62,37 @@ struct cfd_ctx {
   long long max_M = 0;
   long long launches = 0;
   std::string err;
+  // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read
+  bool prof_on = false;
+  std::vector<cudaEvent_t> prof_ev;
+  std::vector<int> prof_id;
+  size_t prof_used = 0;
+};
+
+// kernel classes of cfd_profile_read
+enum ProfClass { PK_INV_XI = 0, PK_INV_ETA, PK_INV_ZETA, PK_VISC_FLUX, PK_VISC_DIV, PK_RK, PK_RES, PK_FILL, PK_BC, PK_METRICS, PK_COPY, PK_OTHER };
+
+// Brackets the launches enqueued during its lifetime with two events when profiling is on.
+struct ProfScope {
+  cfd_ctx* c;
+  cudaEvent_t stop = nullptr;
+  ProfScope(cfd_ctx* ctx, int id) : c(ctx) {
+    if (!c->prof_on) return;
+    if (c->prof_used + 2 > c->prof_ev.size()) {
+      cudaEvent_t a, b;
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+      c->prof_ev.push_back(a);
+      c->prof_ev.push_back(b);
+    }
+    cudaEventRecord(c->prof_ev[c->prof_used], c->stream);
+    stop = c->prof_ev[c->prof_used + 1];
+    c->prof_id.resize(c->prof_ev.size() / 2);
+    c->prof_id[c->prof_used / 2] = id;
+    c->prof_used += 2;
+  }
+  ~ProfScope() {
+    if (stop) cudaEventRecord(stop, c->stream);
+  }
 };
 
 // ---- kernel launchers (each enqueues on ctx->stream and bumps ctx->launches) --------------------

@@ -43,6 +43,7 @@ int launch_fill_connect(cfd_ctx* c, int field) {
     int gx = (int)((mx + 255) / 256);
     if (gx > 2048) gx = 2048;
     dim3 grid(gx, (unsigned)nt);
+    ProfScope ps(c, PK_FILL);
     if (field == 0) k_fill<5, false><<<grid, 256, 0, c->stream>>>(c->d_tasks[p], c->d_blocks, 0);
     else k_fill<3, true><<<grid, 256, 0, c->stream>>>(c->d_tasks[p], c->d_blocks, 1);
     c->launches++;
@@ -85,6 +86,7 @@ int launch_bc_xyz(cfd_ctx* c) {
     const BlockDev& B = c->blk[T.block];
     const int an = T.face / 2;
     const int cells = B.m[(an + 1) % 3] * B.m[(an + 2) % 3];
+    ProfScope ps(c, PK_BC);
     k_bc_xyz<<<(cells + 255) / 256, 256, 0, c->stream>>>(B, T.face, T.type);
     c->launches++;
   }
@@ -186,6 +188,7 @@ int launch_bc_q(cfd_ctx* c) {
     const BlockDev& B = c->blk[T.block];
     const int an = T.face / 2;
     const int cells = (B.n[(an + 1) % 3] + 6) * (B.n[(an + 2) % 3] + 6);
+    ProfScope ps(c, PK_BC);
     k_bc_q<<<(cells + 127) / 128, 128, 0, c->stream>>>(B, c->pd, T.face, T.type);
     c->launches++;
   }
@@ -254,6 +257,7 @@ __global__ void __launch_bounds__(256) k_metric_khat(BlockDev B, const double* _
 
 int launch_metrics(cfd_ctx* c) {
   for (const BlockDev& B : c->blk) {
+    ProfScope ps(c, PK_METRICS);
     k_metric_d1<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, c->ws);
     const long long box = (long long)(B.n[0] + 6) * (B.n[1] + 6) * (B.n[2] + 6);
     k_metric_khat<<<(unsigned)((box + 255) / 256), 256, 0, c->stream>>>(B, c->ws, c->d_flag);
@@ -331,6 +335,7 @@ int launch_rk(cfd_ctx* c, int stage, double dt) {
     long long g = (N + 255) / 256;
     const int cap = rk_max_partial_blocks();
     if (g > cap) g = cap;
+    ProfScope ps(c, PK_RK);
     if (stage == 1) k_rk<1><<<(unsigned)g, 256, 0, c->stream>>>(B, dt, a, b, partials + (long long)used * 5);
     else if (stage == 2) k_rk<2><<<(unsigned)g, 256, 0, c->stream>>>(B, dt, a, b, nullptr);
     else k_rk<3><<<(unsigned)g, 256, 0, c->stream>>>(B, dt, a, b, nullptr);
@@ -338,6 +343,7 @@ int launch_rk(cfd_ctx* c, int stage, double dt) {
     c->launches++;
   }
   if (stage == 1) {
+    ProfScope ps(c, PK_RES);
     k_res_final<<<1, 160, 0, c->stream>>>(partials, used, c->d_res);
     c->launches++;
   }

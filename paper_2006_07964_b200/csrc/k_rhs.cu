@@ -334,24 +334,27 @@ int launch_rhs(cfd_ctx* c) {
     {
       constexpr int T = TileCfg<0>::TS - 2, NL = TileCfg<0>::NL;
       dim3 grid((B.n[0] + T - 1) / T, (B.n[1] + NL - 1) / NL, B.n[2]);
+      ProfScope ps(c, PK_INV_XI);
       k_inviscid<0><<<grid, dim3(TileCfg<0>::TS, NL), 0, c->stream>>>(B, c->pd, 0);
     }
     {
       constexpr int T = TileCfg<1>::TS - 2, NL = TileCfg<1>::NL;
       dim3 grid((B.n[0] + NL - 1) / NL, (B.n[1] + T - 1) / T, B.n[2]);
+      ProfScope ps(c, PK_INV_ETA);
       k_inviscid<1><<<grid, dim3(NL, TileCfg<1>::TS), 0, c->stream>>>(B, c->pd, 1);
     }
     {
       constexpr int T = TileCfg<2>::TS - 2, NL = TileCfg<2>::NL;
       dim3 grid((B.n[0] + NL - 1) / NL, B.n[1], (B.n[2] + T - 1) / T);
+      ProfScope ps(c, PK_INV_ZETA);
       k_inviscid<2><<<grid, dim3(NL, TileCfg<2>::TS), 0, c->stream>>>(B, c->pd, visc ? 3 : 2);
     }
     c->launches += 3;
     if (visc) {
       dim3 g1((B.n[0] + 6 + 127) / 128, B.n[1] + 6, B.n[2] + 6);
-      k_visc_flux<<<g1, 128, 0, c->stream>>>(B, c->pd, c->ws);
+      { ProfScope ps(c, PK_VISC_FLUX); k_visc_flux<<<g1, 128, 0, c->stream>>>(B, c->pd, c->ws); }
       dim3 g2((B.n[0] + 255) / 256, B.n[1], B.n[2]);
-      k_visc_div<<<g2, 256, 0, c->stream>>>(B, c->ws);
+      { ProfScope ps(c, PK_VISC_DIV); k_visc_div<<<g2, 256, 0, c->stream>>>(B, c->ws); }
       c->launches += 2;
     }
   }

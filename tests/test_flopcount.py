@@ -22,3 +22,21 @@ def test_flopcount_runs_and_matches_hand_count():
     assert s2["sqrt"] >= 6 and s2["div"] >= 32
     # the paper's claim for the modified scheme: sharing beta and the characteristic variables "reduces calculation"
     assert out["S2_per_direction_original"]["total"] > 1.3 * s2["total"]
+
+
+def test_bench_constants_equal_the_oracle_count():
+    """bench.py's roofline numerators are the oracle's exact per-point counts (no hand-typed drift)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import build
+
+    build.build()
+    out = json.loads(subprocess.check_output([os.path.join(ROOT, "oracle", "flopcount")]))
+    sys.path.insert(0, ROOT)
+    import bench
+
+    F = bench.FLOPS_PER_POINT
+    assert F["inviscid_dir"] == out["S2_per_direction_modified"]["total"]
+    assert F["viscous"] == out["S3_viscous"]["total"]
+    assert F["rk"] == out["S4_rk_stage"]["total"]
+    assert F["ns_stage"] == out["total_navier_stokes_per_point_stage"]["total"]
+    assert F["euler_stage"] == out["total_euler_per_point_stage"]["total"]

@@ -307,3 +307,49 @@ def test_error_codes(W, B):
     with pytest.raises(B.CfdError) as e:
         g2.load_case(flipped)
     assert e.value.code == -3
+
+
+# ------------------------------------------------------------------------------------------------
+# e2e entry with host buffers (bench.py's e2e leg) and the per-kernel event timing
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["ragged-ns", "multiblock", "cylinder"])
+def test_step_host_matches_oracle_and_device_path(po, W, B, which):
+    import torch
+
+    if which == "ragged-ns":
+        case = ragged_case(W, 1)
+    elif which == "multiblock":
+        case = W.c4_multiblock(nb=10, mach=0.3)
+    else:
+        case = W.c5_cylinder(ni=40, nj=24, nk=10)
+    o, g = pair(po, B, case)
+    dt = o.cfl_dt(0.5)
+    qh = [torch.from_numpy(np.ascontiguousarray(case.q0[b])).pin_memory() for b in range(len(case.dims))]
+    qo = [torch.empty_like(q).pin_memory() for q in qh]
+    rg = g.step_host(qh, qo, dt, want_res=True)
+    ro = o.step(dt)
+    assert np.allclose(rg, ro, rtol=1e-10)
+    for b in range(len(case.dims)):
+        ref = o.interior(b, "q")
+        err = np.abs(qo[b].numpy() - ref).max() / np.abs(ref).max()
+        assert err < 1e-12, (which, b, err)
+        assert np.array_equal(qo[b].numpy(), g.to_numpy(b, "q"))  # D2H copy is the device state, bit for bit
+    # wrong shape / non-contiguous host buffers are refused before any copy
+    with pytest.raises(B.CfdError):
+        g.step_host([q[:, 1:] for q in qh], qo, dt)
+
+
+def test_profile_counts_every_hot_path_launch(po, W, B):
+    case = ragged_case(W, 1)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    g.profile_enable(True)
+    l0 = g.launch_count
+    g.step(1e-3)
+    prof = g.profile_read()
+    assert sum(n for _, n in prof.values()) == g.launch_count - l0
+    assert all(ms >= 0.0 for ms, _ in prof.values())
+    assert any(k.startswith("inviscid") or k.startswith("rhs") or k.startswith("sweep") for k in prof)
+    g.profile_enable(False)
+    g.step(1e-3)
+    assert g.profile_read() == {}
