@@ -85,8 +85,9 @@ typedef struct {
   double* jac;  /* [1][M] J (Eq. 8) */
 } cfd_block_ptrs;
 
-/* Bytes of device scratch the caller must pass to cfd_create_blocks (12 doubles per point of the
- * largest block: viscous point fluxes / metric first derivatives, plus reduction partials). */
+/* Bytes of device scratch the caller must pass to cfd_create_blocks (16 doubles per point of the
+ * largest block: 12 viscous point-flux rows + phi = (u,v,w,T), or the 9 metric first derivatives; plus
+ * reduction partials). */
 size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params* params);
 
 /* Build a context over nblocks point-matched blocks (a patch is a whole block face).
@@ -155,6 +156,12 @@ long long cfd_launch_count(const cfd_ctx*);
  * throughput of the device (the "alu" roofline denominator).  Returns host values (TFLOP/s,
  * FMA = 2 flops) in *tflops; synchronises. */
 int cfd_fp64_peak_probe(int iters, double* tflops);
+
+/* Device self-test of the branch-free fp64 reciprocal / reciprocal square root the hot kernels use instead
+ * of IEEE division (csrc/fastmath.cuh): for n HOST values x > 0 writes 1/x and 1/sqrt(x) as the kernels compute
+ * them into the HOST arrays rcp_out, rsqrt_out (tests compare with correctly rounded results).  Allocates
+ * and frees its own scratch; synchronises.  Not on the hot path. */
+int cfd_selftest_fastmath(int n, const double* x_host, double* rcp_out_host, double* rsqrt_out_host);
 
 #ifdef __cplusplus
 }

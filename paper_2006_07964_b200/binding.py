@@ -19,7 +19,7 @@ ABI_SYMBOLS = (
     "cfd_workspace_bytes", "cfd_create_blocks", "cfd_compute_metrics", "cfd_rhs", "cfd_rk_stage",
     "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
-    "cfd_profile_name",
+    "cfd_profile_name", "cfd_selftest_fastmath",
 )
 PROF_NCLASS = 12
 
@@ -77,6 +77,8 @@ def _load():
     L.cfd_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.cfd_profile_name.restype = C.c_char_p
     L.cfd_profile_name.argtypes = [C.c_int]
+    L.cfd_selftest_fastmath.restype = C.c_int
+    L.cfd_selftest_fastmath.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.cfd_fp64_peak_probe.restype = C.c_int
     L.cfd_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
     return L
@@ -92,6 +94,17 @@ def device_peak_probe(iters=4096):
     if rc != 0:
         raise CfdError(rc, "cfd_fp64_peak_probe failed")
     return t.value
+
+
+def selftest_fastmath(x):
+    """(1/x, 1/sqrt(x)) as the hot kernels compute them (csrc/fastmath.cuh), for a host fp64 array x > 0."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    r, s = np.empty_like(x), np.empty_like(x)
+    dp = C.POINTER(C.c_double)
+    rc = lib.cfd_selftest_fastmath(int(x.size), x.ctypes.data_as(dp), r.ctypes.data_as(dp), s.ctypes.data_as(dp))
+    if rc != 0:
+        raise CfdError(rc, "cfd_selftest_fastmath failed")
+    return r, s
 
 
 class Context:

@@ -9,7 +9,7 @@ static thread_local std::string g_create_err;
 
 static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD_FACE_INTERFACE; }
 
-size_t ws_partials_offset_doubles(long long max_M) { return (size_t)12 * (size_t)max_M; }
+size_t ws_partials_offset_doubles(long long max_M) { return (size_t)16 * (size_t)max_M; }
 int rk_max_partial_blocks() { return 4096; }
 
 extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
@@ -175,6 +175,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   }
   if ((e = cudaMalloc(&c->d_flag, sizeof(int))) != cudaSuccess) return cuda_fail(e, "cudaMalloc flag");
   if ((e = cudaMalloc(&c->d_res, sizeof(double) * 8)) != cudaSuccess) return cuda_fail(e, "cudaMalloc res");
+  if (sweep_init() != 0) return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute (dynamic shared memory of the sweep kernels)");
   *out = c;
   return CFD_OK;
 }
@@ -280,7 +281,7 @@ extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const
   return CFD_OK;
 }
 
-static const char* k_prof_names[CFD_PROF_NCLASS] = {"inviscid_xi", "inviscid_eta", "inviscid_zeta", "visc_flux", "visc_div", "rk_stage",
+static const char* k_prof_names[CFD_PROF_NCLASS] = {"inviscid_xi", "inviscid_eta", "inviscid_zeta", "visc_flux", "visc_phi", "rk_stage",
                                                     "residual_final", "ghost_fill", "phys_bc", "metrics", "host_copy", "other"};
 
 extern "C" const char* cfd_profile_name(int id) { return (id >= 0 && id < CFD_PROF_NCLASS) ? k_prof_names[id] : ""; }
@@ -306,6 +307,11 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
   }
   c->prof_used = 0;
   return CFD_OK;
+}
+
+extern "C" int cfd_selftest_fastmath(int n, const double* x_host, double* rcp_host, double* rsqrt_host) {
+  if (n < 1 || !x_host || !rcp_host || !rsqrt_host) return CFD_E_ARG;
+  return launch_fastmath_selftest(n, x_host, rcp_host, rsqrt_host);
 }
 
 extern "C" int cfd_fp64_peak_probe(int iters, double* tflops) {

@@ -70,7 +70,7 @@ struct cfd_ctx {
 };
 
 // kernel classes of cfd_profile_read
-enum ProfClass { PK_INV_XI = 0, PK_INV_ETA, PK_INV_ZETA, PK_VISC_FLUX, PK_VISC_DIV, PK_RK, PK_RES, PK_FILL, PK_BC, PK_METRICS, PK_COPY, PK_OTHER };
+enum ProfClass { PK_INV_XI = 0, PK_INV_ETA, PK_INV_ZETA, PK_VISC_FLUX, PK_VISC_PHI, PK_RK, PK_RES, PK_FILL, PK_BC, PK_METRICS, PK_COPY, PK_OTHER };
 
 // Brackets the launches enqueued during its lifetime with two events when profiling is on.
 struct ProfScope {
@@ -103,6 +103,8 @@ int launch_metrics(cfd_ctx* c);
 int launch_rhs(cfd_ctx* c);
 int launch_rk(cfd_ctx* c, int stage, double dt);
 int launch_fp64_probe(int iters, double* tflops);
+int launch_fastmath_selftest(int n, const double* x_host, double* rcp_host, double* rsqrt_host);
+int sweep_init();
 
 size_t ws_partials_offset_doubles(long long max_M);
 int rk_max_partial_blocks();

@@ -1,6 +1,7 @@
 // Kernels for S1 (metrics/Jacobian), S4 (RK stage + residual), S5 (physical BCs), S6 (ghost fill),
 // and the FP64 peak probe.  sm_100a, fp64.  P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.
 #include "cfd_internal.cuh"
+#include "fastmath.cuh"
 
 // =================================================================================================
 // S6: ghost fill through signed index permutations (U15; P:L262 bc_block, "on GPU without
@@ -394,4 +395,29 @@ int launch_fp64_probe(int iters, double* tflops) {
   cudaFree(d);
   *tflops = best;
   return CFD_OK;
+}
+
+// =================================================================================================
+// Self-test of fastmath.cuh (cfd_selftest_fastmath).
+// =================================================================================================
+__global__ void k_fastmath(int n, const double* __restrict__ x, double* __restrict__ r, double* __restrict__ s) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  r[t] = frcp(x[t]);
+  s[t] = frsqrt(x[t]);
+}
+
+int launch_fastmath_selftest(int n, const double* xh, double* rh, double* sh) {
+  double* d = nullptr;
+  const size_t nb = sizeof(double) * (size_t)n;
+  if (cudaMalloc(&d, 3 * nb) != cudaSuccess) return CFD_E_CUDA;
+  int rc = CFD_OK;
+  if (cudaMemcpy(d, xh, nb, cudaMemcpyHostToDevice) != cudaSuccess) rc = CFD_E_CUDA;
+  if (rc == CFD_OK) {
+    k_fastmath<<<(n + 255) / 256, 256>>>(n, d, d + n, d + 2 * (size_t)n);
+    if (cudaMemcpy(rh, d + n, nb, cudaMemcpyDeviceToHost) != cudaSuccess) rc = CFD_E_CUDA;
+    if (rc == CFD_OK && cudaMemcpy(sh, d + 2 * (size_t)n, nb, cudaMemcpyDeviceToHost) != cudaSuccess) rc = CFD_E_CUDA;
+  }
+  cudaFree(d);
+  return rc;
 }

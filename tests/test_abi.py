@@ -41,8 +41,8 @@ def test_workspace_bytes_is_pure_host_arithmetic(lib):
     p = lib._Params()
     got = lib.lib.cfd_workspace_bytes(2, d, C.byref(p))
     M = 44 ** 3
-    assert got >= 12 * M * 8
-    assert got < 13 * M * 8 + (1 << 20)
+    assert got >= 16 * M * 8
+    assert got < 17 * M * 8 + (1 << 20)
 
 
 def test_no_cuda_device_fails_loudly(lib):

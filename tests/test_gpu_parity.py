@@ -93,6 +93,19 @@ def ragged_case(W, viscous=1):
                   W.default_params(viscous=viscous, mach=0.4, reynolds=300.0), dt=1e-3, steps=0)
 
 
+def test_fastmath_accuracy(B):
+    """csrc/fastmath.cuh (MUFU seed + one cubic Newton step) against correctly rounded 1/x and 1/sqrt(x) over the
+    magnitudes the kernels feed it (rho, c^2, |khat|^2 ~ 1e-6..1e6; WENO denominators down to (4 eps)^8 ~ 1e-43)."""
+    rng = np.random.default_rng(5)
+    x = np.concatenate([rng.uniform(0.5, 2.0, 20000), 10.0 ** rng.uniform(-45, 40, 20000), [1.0, 2.0, 4.0, 0.25, 3.0]])
+    r, s = B.selftest_fastmath(x)
+    exact_r = (1.0 / x.astype(np.longdouble))
+    exact_s = 1.0 / np.sqrt(x.astype(np.longdouble))
+    er = np.abs((r - exact_r) / exact_r).max()
+    es = np.abs((s - exact_s) / exact_s).max()
+    assert er < 4.5e-16 and es < 4.5e-16, (float(er), float(es))  # <= 2 ulp
+
+
 # ------------------------------------------------------------------------------------------------
 # S2 + S3: RHS parity, element by element
 # ------------------------------------------------------------------------------------------------
