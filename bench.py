@@ -236,7 +236,7 @@ def dominant_roofline(prof, case, n_steps, hbm_gbs, hbm_src, dfma_probe_tflops, 
     }
 
 
-def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True):
+def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, plan=0):
     import torch
 
     from paper_2006_07964_b200 import binding as B
@@ -244,6 +244,8 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True):
     case = make_case(name)
     ctx = B.Context(case.dims, case.faces, case.params, device=device)
     ctx.load_case(case)
+    if plan:
+        ctx.set_sweep_plan(plan)
     pts = case.npoints
     dt = case.dt
     torch.cuda.synchronize(device)
@@ -339,7 +341,7 @@ def run_ours(args):
 
     hbm_gbs, hbm_src = load_peaks()
     probe = B.device_peak_probe(2048)
-    main = measure_gpu(args.workload, args.steps, args.warmup, device, dist=dist, e2e=True, profile=True)
+    main = measure_gpu(args.workload, args.steps, args.warmup, device, dist=dist, e2e=True, profile=True, plan=args.plan)
     case, pts = main["case"], main["pts"]
     visc = int(case.params["viscous"])
     n_stage = 3 * args.steps
@@ -412,6 +414,7 @@ def main():
     ap.add_argument("--workload", default="sweep256", choices=sorted(WORKLOADS))
     ap.add_argument("--also", default="c3,c4,c5", help="comma list of extra workloads measured briefly (N=1 only)")
     ap.add_argument("--no-also", action="store_true")
+    ap.add_argument("--plan", type=int, default=0, help="cfd_set_sweep_plan (0 default; 1 all tiled; 2 all marching)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     if args.impl == "reference":

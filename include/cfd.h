@@ -157,6 +157,12 @@ long long cfd_launch_count(const cfd_ctx*);
  * FMA = 2 flops) in *tflops; synchronises. */
 int cfd_fp64_peak_probe(int iters, double* tflops);
 
+/* Kernel plan of the three inviscid sweeps inside cfd_rhs (all plans compute the same R up to summation order):
+ *   0 (default) xi as a tiled sweep (one thread per point), then eta and zeta as marching sweeps (one thread walks
+ *     a grid line segment; Q, khat staged once per point through a thread-private shared-memory ring);
+ *   1 all three tiled;   2 all three marching (the xi march reads with stride: for measurement). */
+int cfd_set_sweep_plan(cfd_ctx*, int plan);
+
 /* Device self-test of the branch-free fp64 reciprocal / reciprocal square root the hot kernels use instead
  * of IEEE division (csrc/fastmath.cuh): for n HOST values x > 0 writes 1/x and 1/sqrt(x) as the kernels compute
  * them into the HOST arrays rcp_out, rsqrt_out (tests compare with correctly rounded results).  Allocates

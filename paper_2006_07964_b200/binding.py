@@ -19,7 +19,7 @@ ABI_SYMBOLS = (
     "cfd_workspace_bytes", "cfd_create_blocks", "cfd_compute_metrics", "cfd_rhs", "cfd_rk_stage",
     "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
-    "cfd_profile_name", "cfd_selftest_fastmath",
+    "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan",
 )
 PROF_NCLASS = 12
 
@@ -77,6 +77,8 @@ def _load():
     L.cfd_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.cfd_profile_name.restype = C.c_char_p
     L.cfd_profile_name.argtypes = [C.c_int]
+    L.cfd_set_sweep_plan.restype = C.c_int
+    L.cfd_set_sweep_plan.argtypes = [C.c_void_p, C.c_int]
     L.cfd_selftest_fastmath.restype = C.c_int
     L.cfd_selftest_fastmath.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.cfd_fp64_peak_probe.restype = C.c_int
@@ -241,6 +243,9 @@ class Context:
         if not ok:
             raise CfdError(-1, f"step_host: block {b} needs a C-contiguous host fp64 array of shape (5,{nk},{nj},{ni})")
         return ptr
+
+    def set_sweep_plan(self, plan):
+        self._chk(lib.cfd_set_sweep_plan(self.h, int(plan)))
 
     def profile_enable(self, on=True):
         self._chk(lib.cfd_profile_enable(self.h, 1 if on else 0))

@@ -309,6 +309,13 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
   return CFD_OK;
 }
 
+extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
+  if (!c) return CFD_E_ARG;
+  if (plan < 0 || plan > 2) { c->err = "cfd_set_sweep_plan: plan must be 0, 1 or 2"; return CFD_E_ARG; }
+  c->sweep_plan = plan;
+  return CFD_OK;
+}
+
 extern "C" int cfd_selftest_fastmath(int n, const double* x_host, double* rcp_host, double* rsqrt_host) {
   if (n < 1 || !x_host || !rcp_host || !rsqrt_host) return CFD_E_ARG;
   return launch_fastmath_selftest(n, x_host, rcp_host, rsqrt_host);

@@ -61,6 +61,7 @@ struct cfd_ctx {
   size_t ws_bytes = 0;
   long long max_M = 0;
   long long launches = 0;
+  int sweep_plan = 0;                 // cfd_set_sweep_plan
   std::string err;
   // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read
   bool prof_on = false;

@@ -22,7 +22,7 @@
 //  * alpha_k = 1/(eps+beta_k)^2 replaced by the product of the other two (eps+beta)^2 (common denominator),
 //    all three scaled by 4 (cancels in the ratio), one reciprocal for both normalisations.
 #include "cfd_internal.cuh"
-#include "fastmath.cuh"
+#include "sweep_math.cuh"
 
 namespace {
 
@@ -33,70 +33,6 @@ struct SweepCfg {
   static constexpr int TE = TS + 4;              // point-flux slots: positions -3 .. TS relative to the first output
   static constexpr size_t smem_doubles(bool visc) { return (size_t)15 * TS * NL + (size_t)(visc ? 9 : 5) * TE * NL; }
 };
-
-// Eqs. 14-17 on the projected differences D1..D4 of one characteristic field; eps4 = 4 eps.
-__device__ __forceinline__ void weno_corr(double D1, double D2, double D3, double D4, double eps4, double& cL, double& cR) {
-  const double t1 = D2 - D1, t3 = D3 - D2, t5 = D4 - D3;
-  const double t2 = fma(3.0, D2, -D1), t4 = D2 + D3, t6 = fma(-3.0, D3, D4);
-  const double dA = fma((13.0 / 3.0) * t1, t1, fma(t2, t2, eps4));  // 4 (eps + beta_1)
-  const double dB = fma((13.0 / 3.0) * t3, t3, fma(t4, t4, eps4));
-  const double dC = fma((13.0 / 3.0) * t5, t5, fma(t6, t6, eps4));
-  const double pA = dB * dC, pB = dA * dC, pC = dA * dB;
-  const double sA = pA * pA, sB = (10.0 * pB) * pB, sC = pC * pC;  // 16 gamma_k alpha_k (dA dB dC)^2
-  const double g1 = t1 - t3, g2 = t5 - t3;
-  const double x = sA * g1, y = sC * g2;
-  const double denL = fma(5.0, sC, sA + sB), denR = fma(5.0, sA, sB + sC);
-  const double numL = fma(0.375, x, -0.625 * y), numR = fma(0.375, y, -0.625 * x);
-  const double inv = frcp(denL * denR);
-  cL = (numL * denR) * inv;
-  cR = (numR * denL) * inv;
-}
-
-// Steger–Warming split flux (U3) of state U through the interface metric (kx,ky,kz), kn = |k|, ikn = 1/|k|.
-template <int SGN>
-__device__ __forceinline__ void sw_flux(const double U[5], double kx, double ky, double kz, double kn, double ikn,
-                                        double gamma, double F[5]) {
-  const double g1 = gamma - 1.0;
-  const double ir = frcp(U[0]);
-  const double u = U[1] * ir, v = U[2] * ir, w = U[3] * ir;
-  const double q2 = fma(u, u, fma(v, v, w * w));
-  const double p = g1 * fma(-0.5 * U[0], q2, U[4]);
-  const double c2 = (gamma * p) * ir;
-  const double c = c2 * frsqrt(c2);
-  const double th = fma(kx, u, fma(ky, v, kz * w));
-  const double ck = c * kn;
-  double l1 = th, l4 = th + ck, l5 = th - ck;
-  if (SGN > 0) { l1 = fmax(l1, 0.0); l4 = fmax(l4, 0.0); l5 = fmax(l5, 0.0); }  // (l + |l|)/2 exactly
-  else { l1 = fmin(l1, 0.0); l4 = fmin(l4, 0.0); l5 = fmin(l5, 0.0); }
-  const double a1 = (2.0 * g1) * l1, s45 = l4 + l5, d45 = l4 - l5;
-  const double f = U[0] * (0.5 / gamma);
-  const double fA = f * (a1 + s45), fc = f * ((c * ikn) * d45);
-  F[0] = fA;
-  F[1] = fma(fA, u, fc * kx);
-  F[2] = fma(fA, v, fc * ky);
-  F[3] = fma(fA, w, fc * kz);
-  // 0.5 a1 q2 + 0.5 s45 (q2 + c2) + cn th + (3-g)/(2(g-1)) s45 c2  =  q2/2 (a1+s45) + cn th + s45 c2/(g-1)
-  F[4] = fma(0.5 * q2, fA, fma(fc, th, ((f * s45) * c2) * (1.0 / g1)));
-}
-
-__device__ __forceinline__ double khalf(double m2, double m1, double z0, double p1, double p2, double p3) {
-  // U5: symmetric 6-point Lagrange (150, -25, 3)/256
-  return fma(150.0 / 256.0, z0 + p1, fma(-25.0 / 256.0, m1 + p2, (3.0 / 256.0) * (m2 + p3)));
-}
-
-// Eq. 4 from conservative state
-__device__ __forceinline__ void point_flux(double r, double m1, double m2, double m3, double e, double kx, double ky, double kz,
-                                           double gamma, double F[5]) {
-  const double ir = frcp(r);
-  const double u = m1 * ir, v = m2 * ir, w = m3 * ir;
-  const double p = (gamma - 1.0) * fma(-0.5 * r, fma(u, u, fma(v, v, w * w)), e);
-  const double th = fma(kx, u, fma(ky, v, kz * w));
-  F[0] = r * th;
-  F[1] = fma(m1, th, kx * p);
-  F[2] = fma(m2, th, ky * p);
-  F[3] = fma(m3, th, kz * p);
-  F[4] = (e + p) * th;
-}
 
 // ACC 0: r = X;  1: r += X;  2: r = J (r + X)   with X = dFv/dxi^d - D^d   (U18 up to summation order)
 template <int DIR, int ACC, bool VISC>
@@ -298,6 +234,9 @@ void launch_one(cfd_ctx* c, const BlockDev& B, bool visc) {
 
 }  // namespace
 
+int march_init();
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc);
+
 int sweep_init() {
   // opt in to > 48 KB of dynamic shared memory
   cudaError_t e = cudaSuccess;
@@ -308,14 +247,27 @@ int sweep_init() {
                                                  (int)(SweepCfg<D>::smem_doubles(false) * sizeof(double)));
   OPT(0, 0) OPT(1, 1) OPT(2, 2)
 #undef OPT
-  return e == cudaSuccess ? 0 : -1;
+  if (e != cudaSuccess) return -1;
+  return march_init();
 }
 
+// Sweep plans (cfd_set_sweep_plan): 0 = xi tiled and first (plain store), eta and zeta marching (zeta applies J);
+// 1 = all three tiled (one thread per point);  2 = all three marching (xi lanes run along j: uncoalesced).
 int launch_sweeps(cfd_ctx* c, const BlockDev& B) {
   const bool visc = c->pd.viscous != 0;
-  { ProfScope ps(c, PK_INV_XI); launch_one<0, 0>(c, B, visc); }
-  { ProfScope ps(c, PK_INV_ETA); launch_one<1, 1>(c, B, visc); }
-  { ProfScope ps(c, PK_INV_ZETA); launch_one<2, 2>(c, B, visc); }
-  c->launches += 3;
+  if (c->sweep_plan == 1) {
+    { ProfScope ps(c, PK_INV_XI); launch_one<0, 0>(c, B, visc); }
+    { ProfScope ps(c, PK_INV_ETA); launch_one<1, 1>(c, B, visc); }
+    { ProfScope ps(c, PK_INV_ZETA); launch_one<2, 2>(c, B, visc); }
+    c->launches += 3;
+  } else if (c->sweep_plan == 2) {
+    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 0); }
+    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 1); }
+    { ProfScope ps(c, PK_INV_XI); launch_march(c, B, 0, 2); }
+  } else {
+    { ProfScope ps(c, PK_INV_XI); launch_one<0, 0>(c, B, visc); c->launches++; }
+    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1); }
+    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 2); }
+  }
   return 0;
 }

@@ -122,6 +122,21 @@ def test_rhs_parity(po, W, B, which):
     assert_rhs_parity(o, g, case)
 
 
+@pytest.mark.parametrize("plan", [1, 2])
+@pytest.mark.parametrize("which", ["ragged-ns", "ragged-euler", "multiblock-ns", "cylinder-ns", "tiny"])
+def test_rhs_parity_other_sweep_plans(po, W, B, which, plan):
+    """cfd_set_sweep_plan: all-tiled (1) and all-marching (2) sweeps against the oracle (plan 0 is the default
+    everywhere else)."""
+    case = {"ragged-ns": lambda: ragged_case(W, 1),
+            "ragged-euler": lambda: ragged_case(W, 0),
+            "multiblock-ns": lambda: W.c4_multiblock(nb=12, mach=0.3),
+            "cylinder-ns": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0, noise=1e-2),
+            "tiny": lambda: W.tgv_sine_box(6, viscous=1, mach=0.3)}[which]()
+    o, g = pair(po, B, case)
+    g.set_sweep_plan(plan)
+    assert_rhs_parity(o, g, case)
+
+
 def test_rhs_parity_strong_gradients(po, W, B):
     """Non-smooth data (the WENO weights far from the linear ones): seeded random +-20 % perturbation per node."""
     case = W.c1_vortex(24)
