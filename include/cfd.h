@@ -158,9 +158,10 @@ long long cfd_launch_count(const cfd_ctx*);
 int cfd_fp64_peak_probe(int iters, double* tflops);
 
 /* Kernel plan of the three inviscid sweeps inside cfd_rhs (all plans compute the same R up to summation order):
- *   0 (default) xi as a tiled sweep (one thread per point), then eta and zeta as marching sweeps (one thread walks
- *     a grid line segment; Q, khat staged once per point through a thread-private shared-memory ring);
- *   1 all three tiled;   2 all three marching (the xi march reads with stride: for measurement). */
+ *   0 (default) all three as marching sweeps (one thread walks a grid line segment; Q, khat staged once per point
+ *     through shared memory); the xi sweep stages aligned 4-point chunks of 32 lines per warp (transposed staging);
+ *   1 all three tiled (one thread per point);   2 all three with the plain marching kernel (the xi march reads with
+ *     stride: for measurement);   3 xi tiled, eta and zeta marching. */
 int cfd_set_sweep_plan(cfd_ctx*, int plan);
 
 /* Device self-test of the branch-free fp64 reciprocal / reciprocal square root the hot kernels use instead

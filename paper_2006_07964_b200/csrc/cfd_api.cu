@@ -311,7 +311,7 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
 
 extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
   if (!c) return CFD_E_ARG;
-  if (plan < 0 || plan > 2) { c->err = "cfd_set_sweep_plan: plan must be 0, 1 or 2"; return CFD_E_ARG; }
+  if (plan < 0 || plan > 3) { c->err = "cfd_set_sweep_plan: plan must be 0..3"; return CFD_E_ARG; }
   c->sweep_plan = plan;
   return CFD_OK;
 }

@@ -16,10 +16,14 @@
 //    (3/4, -3/20, 1/60).  Exact identity; only the summation order differs from Eq. 19 as printed.
 #include "cfd_internal.cuh"
 #include "sweep_math.cuh"
+#include <cmath>
 
 namespace {
 
 constexpr int MT = 128;     // threads per CTA
+#ifndef MINB
+#define MINB 2
+#endif
 constexpr int RING = 8;     // ring slots (positions j-3 .. j+3 live, one spare)
 constexpr int RV = 8;       // doubles per slot: Q (5) + khat^d (3)
 
@@ -28,6 +32,7 @@ struct MarchArgs {
   const double* kh;     // khat^d, + interior origin
   const double* W;      // viscous flux rows of direction d, + interior origin (VISC)
   const double* jac;    // + interior origin (ACC 2)
+  const double* Sx;     // d(Fv^xi)/d(xi) rows from k_visc_flux<true>, + interior origin, or null (added to r when ACC >= 1)
   double* r;            // + interior origin
   long long M;          // plane stride between variables
   long long sl, sm, st; // strides: neighbouring lane, one step along the sweep, third index
@@ -72,8 +77,8 @@ __device__ __forceinline__ double fir_push2(double acc[5], double x, double xv) 
 }
 
 // ACC 0: r = X;  1: r += X;  2: r = J (r + X)   with X = dFv/dxi^d - D^d = -(Phi_{j+1/2} - Phi_{j-1/2})
-template <int ACC, bool VISC>
-__global__ void __launch_bounds__(MT, 2) k_march(MarchArgs A) {
+template <int ACC, bool VISC, bool SX>
+__global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
   extern __shared__ double ring[];  // [RING][RV][MT], thread-private columns
   const int tid = threadIdx.x;
   const long long L = (long long)blockIdx.x * MT + tid;
@@ -138,6 +143,10 @@ __global__ void __launch_bounds__(MT, 2) k_march(MarchArgs A) {
     if (ACC >= 1 && j > p0) {
 #pragma unroll
       for (int m = 0; m < 5; ++m) rold[m] = r[m * M + (long long)(j - 1) * sm];
+      if (SX) {
+#pragma unroll
+        for (int m = 1; m < 5; ++m) rold[m] += A.Sx[base + (long long)(m - 1) * M + (long long)(j - 1) * sm];
+      }
       if (ACC == 2) jac = A.jac[base + (long long)(j - 1) * sm];
     }
     cp_wait<1>();
@@ -196,13 +205,255 @@ __global__ void __launch_bounds__(MT, 2) k_march(MarchArgs A) {
 }
 
 
+
+// ---------------------------------------------------------------------------------------------------------
+// The xi sweep as a marching sweep with WARP-PRIVATE TRANSPOSED STAGING.  Marching along i puts the lanes of a warp
+// on neighbouring j lines (stride m0 doubles): a per-lane load would use 8 of every 32-byte sector.  Instead the warp
+// loads, for its 32 lines, aligned chunks of 4 consecutive i positions (one full 32-byte sector per line and
+// variable; lane -> (line l/4 + 8t, position l%4)) with cp.async into a per-line ring in shared memory (line stride
+// odd: the consumer's reads, all lanes at the same offset, are conflict-free), and every lane then marches along its
+// own line out of shared memory exactly like k_march.  Nothing crosses warps: only __syncwarp.
+//   ring per line: Q (5) + khat^xi (3) x XR = 10 positions, viscous rows (4) x XW = 5 positions -> 100 doubles (+1 pad);
+//   chunk [c, c+4) is issued at step j = c-3 (its slots, positions c-10..c-7, died at step c-4) and awaited at c-2.
+// The output of step j (r at position j-1) is parked in the Q slots of position j-3 (dead: Q is read at j-2..j+2 only)
+// and written out by the same lane mapping as the loads, four positions = one full sector per line at a time, just
+// before those slots are refilled; the flush applies the accumulation mode (r = X, r += X, r = J (r + X)).
+constexpr int XR = 10, XW = 5;
+constexpr int XLS = 8 * XR + 4 * XW + 1;  // 101 doubles per line
+constexpr int XWARPS = 4;
+
+struct XiArgs {
+  const double* q;      // + interior origin
+  const double* kh;
+  const double* W;
+  const double* jac;
+  double* r;
+  long long M;          // plane stride between variables
+  long long sl, st;     // strides: neighbouring line (lane axis), third index; the sweep runs along stride 1
+  int nl, nt, n, S;     // lines, third extent, sweep length, segment length
+  int nlb;              // number of 32-line groups per third index
+  int ph;               // chunk phase: chunk starts c = ph (mod 4) are 32-byte aligned in memory
+  double gamma, eps4;
+};
+
+__device__ __forceinline__ int wrap10(int s) { return s >= XR ? s - XR : s; }
+
+template <int ACC, bool VISC>
+__global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
+  extern __shared__ double ring[];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const long long unit = (long long)blockIdx.x * XWARPS + wid;
+  const int lb = (int)(unit % A.nlb);
+  const long long it = unit / A.nlb;
+  if (it >= A.nt) return;  // warp-uniform; no CTA barriers in this kernel
+  const int p0 = blockIdx.y * A.S;
+  const int p1 = min(A.n, p0 + A.S);
+  double* const wbase = ring + wid * (32 * XLS);
+  double* const my = wbase + lane * XLS;
+  const int l0 = lb * 32;
+  const long long M = A.M;
+  const double gamma = A.gamma, eps4 = A.eps4;
+  // loader / flusher role of this lane: lines l0 + lsub + 8t (t = 0..3), position (chunk start) + lpos
+  const int lsub = lane >> 2, lpos = lane & 3;
+  const long long tbase = it * A.st;
+  long long goff[4];
+  bool lok[4];
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const int ln = l0 + lsub + 8 * t;
+    lok[t] = ln < A.nl;
+    goff[t] = tbase + (long long)min(ln, A.nl - 1) * A.sl;
+  }
+  double* const lbase = wbase + lsub * XLS;  // + t * 8 * XLS
+  const int qlo = p0 - 4, qhi = p1 + 2, wlo = p0 + 1;
+
+  auto load_chunk = [&](int c) {
+    const int pos = c + lpos;
+    if (pos >= qlo && pos <= qhi) {
+      const int s = (pos + 2 * XR) % XR;
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        double* d = lbase + t * 8 * XLS + s;
+        const double* gq = A.q + goff[t] + pos;
+        const double* gk = A.kh + goff[t] + pos;
+#pragma unroll
+        for (int m = 0; m < 5; ++m) cp8(d + m * XR, gq + m * M);
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) cp8(d + (5 + cc) * XR, gk + cc * M);
+      }
+      if (VISC && pos >= wlo) {
+        const int s5 = (pos + 2 * XW) % XW;
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          double* d = lbase + t * 8 * XLS + 8 * XR + s5;
+          const double* gw = A.W + goff[t] + pos;
+#pragma unroll
+          for (int m = 0; m < 4; ++m) cp8(d + m * XW, gw + m * M);
+        }
+      }
+    }
+  };
+  // write out the parked outputs of r positions g .. g+3 (parked in the Q slots of positions g-2 .. g+1)
+  auto flush = [&](int g) {
+    const int pos = g + lpos;
+    if (pos >= p0 && pos < p1) {
+      const int s = (pos - 2 + 2 * XR) % XR;
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        if (!lok[t]) continue;
+        const double* sX = lbase + t * 8 * XLS + s;
+        double* gr = A.r + goff[t] + pos;
+        double jac = 0.0;
+        if (ACC == 2) jac = A.jac[goff[t] + pos];
+#pragma unroll
+        for (int m = 0; m < 5; ++m) {
+          const double X = sX[m * XR];
+          if (ACC == 0) gr[m * M] = X;
+          else if (ACC == 1) gr[m * M] = gr[m * M] + X;
+          else gr[m * M] = jac * (gr[m * M] + X);
+        }
+      }
+    }
+  };
+
+  // ---- prologue: every chunk that starts at or before p0+1 (positions < p0-4 masked out) ----
+  {
+    int c = p0 - 4;
+    c -= ((c - A.ph) & 3);  // align down to the chunk phase
+    for (; c <= p0 + 1; c += 4) load_chunk(c);
+    cp_commit();
+  }
+  double acc[5][5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m)
+#pragma unroll
+    for (int t = 0; t < 5; ++t) acc[m][t] = 0.0;
+  const long long myoff = tbase + (long long)min(l0 + lane, A.nl - 1) * A.sl;
+  double wpro[4][4];
+  if (VISC) {  // the four viscous rows that prime the FIR: read directly (once per segment)
+#pragma unroll
+    for (int t = 0; t < 4; ++t)
+#pragma unroll
+      for (int m = 0; m < 4; ++m) wpro[t][m] = A.W[myoff + (long long)m * M + (p0 - 3 + t)];
+  }
+  cp_wait<0>();
+  __syncwarp();
+  int s0 = (p0 - 1 - 3 + 2 * XR) % XR;  // slot of position j-3 at the first step j = p0-1
+  int w5 = (p0 - 1 + 2 + 2 * XW) % XW;  // slot of W at position j+2
+  // prime the FIR with the point fluxes of p0-3 .. p0 (slots s0+1 .. s0+4)
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const double* s = my + wrap10(s0 + 1 + t);
+    double F[5];
+    point_flux(s[0], s[XR], s[2 * XR], s[3 * XR], s[4 * XR], s[5 * XR], s[6 * XR], s[7 * XR], gamma, F);
+    fir_push(acc[0], F[0]);
+#pragma unroll
+    for (int m = 1; m < 5; ++m) {
+      if (VISC) fir_push2(acc[m], F[m], wpro[t][m - 1]);
+      else fir_push(acc[m], F[m]);
+    }
+  }
+  double ULc[5] = {0, 0, 0, 0, 0}, Phip[5] = {0, 0, 0, 0, 0};
+  for (int j = p0 - 1; j <= p1; ++j) {
+    if (((j + 3 - A.ph) & 3) == 0) {  // chunk c = j+3: flush the outputs parked in its slots, then refill them
+      __syncwarp();
+      flush(j + 3 - 8);
+      load_chunk(j + 3);
+      cp_commit();
+    } else if (((j + 2 - A.ph) & 3) == 0) {
+      cp_wait<0>();
+      __syncwarp();
+    }
+    const double* sl0 = my + s0;
+    const double* sl1 = my + wrap10(s0 + 1);
+    const double* sl2 = my + wrap10(s0 + 2);
+    const double* sl3 = my + wrap10(s0 + 3);
+    const double* sl4 = my + wrap10(s0 + 4);
+    const double* sl5 = my + wrap10(s0 + 5);
+    // ---- point j: U^L_{j+1/2}, U^R_{j-1/2} ----
+    double Qs[5][5], UL[5], UR[5], Fc[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      Qs[0][m] = sl1[m * XR]; Qs[1][m] = sl2[m * XR]; Qs[2][m] = sl3[m * XR]; Qs[3][m] = sl4[m * XR]; Qs[4][m] = sl5[m * XR];
+    }
+    afweno_states(Qs, sl3[5 * XR], sl3[6 * XR], sl3[7 * XR], gamma, eps4, UL, UR, Fc);
+    // ---- FIR: push the point flux of j+2; output = central + viscous part of Phi_{j-1/2} ----
+    double G[5];
+    {
+      double F[5];
+      point_flux(Qs[4][0], Qs[4][1], Qs[4][2], Qs[4][3], Qs[4][4], sl5[5 * XR], sl5[6 * XR], sl5[7 * XR], gamma, F);
+      G[0] = fir_push(acc[0], F[0]);
+      const double* sw = my + 8 * XR + w5;
+#pragma unroll
+      for (int m = 1; m < 5; ++m) G[m] = VISC ? fir_push2(acc[m], F[m], sw[(m - 1) * XW]) : fir_push(acc[m], F[m]);
+    }
+    if (j >= p0) {
+      // ---- interface j-1/2: metric (U5), both split fluxes, numerical flux ----
+      const double kx = khalf(sl0[5 * XR], sl1[5 * XR], sl2[5 * XR], sl3[5 * XR], sl4[5 * XR], sl5[5 * XR]);
+      const double ky = khalf(sl0[6 * XR], sl1[6 * XR], sl2[6 * XR], sl3[6 * XR], sl4[6 * XR], sl5[6 * XR]);
+      const double kz = khalf(sl0[7 * XR], sl1[7 * XR], sl2[7 * XR], sl3[7 * XR], sl4[7 * XR], sl5[7 * XR]);
+      const double kk = fma(kx, kx, fma(ky, ky, kz * kz));
+      const double ikn = frsqrt(kk), kn = kk * ikn;
+      double Fp[5], Fm[5];
+      sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
+      sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+      double* park = my + s0;  // Q slots of position j-3
+#pragma unroll
+      for (int m = 0; m < 5; ++m) {
+        const double Phi = (Fp[m] + Fm[m]) + G[m];
+        if (j > p0) park[m * XR] = Phip[m] - Phi;
+        Phip[m] = Phi;
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < 5; ++m) ULc[m] = UL[m];
+    s0 = wrap10(s0 + 1);
+    w5 = w5 + 1 >= XW ? 0 : w5 + 1;
+  }
+  // ---- flush what is still parked: groups after the last one flushed in the loop ----
+  __syncwarp();
+  {
+    // in-loop flushes covered groups g = j+3-8 for the issue steps j <= p1, i.e. g <= p1-5 on the chunk phase
+    int g = p1 - 5;
+    g -= ((g - A.ph) & 3);  // last group flushed in the loop (or earlier than any output)
+    for (g += 4; g < p1; g += 4) flush(g);
+  }
+}
+
+template <int ACC>
+void launch_march_xi_t(cfd_ctx* c, const XiArgs& A, bool visc) {
+  const long long units = (long long)A.nlb * A.nt;
+  dim3 grid((unsigned)((units + XWARPS - 1) / XWARPS), (unsigned)((A.n + A.S - 1) / A.S));
+  const size_t smem = sizeof(double) * XWARPS * 32 * XLS;
+  if (visc) k_march_xi<ACC, true><<<grid, 32 * XWARPS, smem, c->stream>>>(A);
+  else k_march_xi<ACC, false><<<grid, 32 * XWARPS, smem, c->stream>>>(A);
+}
+
+// Segment count along the sweep: enough CTAs to fill 148 SMs x 2 resident CTAs, as few partial waves as possible,
+// segments of at least 16 points (each segment repeats ~1.5 steps of prologue work).
+int pick_segments(long long ctas_per_seg, int n) {
+  const int maxseg = n / 16 > 0 ? n / 16 : 1;
+  const double slots = 148.0 * 2.0;
+  int best = 1;
+  double best_eff = -1.0;
+  for (int ns = 1; ns <= maxseg; ++ns) {
+    const int S = (n + ns - 1) / ns;
+    const int nseg = (n + S - 1) / S;
+    const double waves = (double)(ctas_per_seg * nseg) / slots;
+    const double eff = waves / ceil(waves) * ((double)n / (double)(nseg * (S + 1.5)));
+    if (eff > best_eff + 1e-9) { best_eff = eff; best = ns; }
+  }
+  return best;
+}
+
 template <int ACC>
 void launch_march_t(cfd_ctx* c, const MarchArgs& A, bool visc) {
   const long long lanes = (long long)A.nl * A.nt;
   dim3 grid((unsigned)((lanes + MT - 1) / MT), (unsigned)((A.n + A.S - 1) / A.S));
   const size_t smem = sizeof(double) * RING * RV * MT;
-  if (visc) k_march<ACC, true><<<grid, MT, smem, c->stream>>>(A);
-  else k_march<ACC, false><<<grid, MT, smem, c->stream>>>(A);
+  if (visc && A.Sx != nullptr && ACC == 1) k_march<1, true, true><<<grid, MT, smem, c->stream>>>(A);
+  else if (visc) k_march<ACC, true, false><<<grid, MT, smem, c->stream>>>(A);
+  else k_march<ACC, false, false><<<grid, MT, smem, c->stream>>>(A);
 }
 
 }  // namespace
@@ -211,15 +462,22 @@ int march_init() {
   cudaError_t e = cudaSuccess;
   const int smem = (int)(sizeof(double) * RING * RV * MT);
 #define OPT(A)                                                                                                      \
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<A, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<A, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<A, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<A, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   OPT(0) OPT(1) OPT(2)
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 #undef OPT
+  const int smx = (int)(sizeof(double) * XWARPS * 32 * XLS);
+#define OPTX(A)                                                                                                        \
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi<A, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx); \
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi<A, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
+  OPTX(0) OPTX(1) OPTX(2)
+#undef OPTX
   return e == cudaSuccess ? 0 : -1;
 }
 
 // One marching sweep of block B along dir (0 xi, 1 eta, 2 zeta) with accumulation mode acc.
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc) {
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, bool sx) {
   const bool visc = c->pd.viscous != 0;
   const long long o0 = B.idx(0, 0, 0);
   MarchArgs A;
@@ -227,25 +485,49 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc) {
   A.kh = B.khat + (long long)(dir * 3) * B.M + o0;
   A.W = visc ? c->ws + (long long)(dir * 4) * B.M + o0 : nullptr;
   A.jac = B.jac + o0;
+  A.Sx = visc && sx ? c->ws + o0 : nullptr;
   A.r = B.r + o0;
   A.M = B.M;
   const int la = dir == 0 ? 1 : 0;                   // lane axis: i, except for the xi sweep (j)
   const int ta = dir == 2 ? 1 : 2;                   // third axis
   A.sl = B.s[la]; A.sm = B.s[dir]; A.st = B.s[ta];
   A.nl = B.n[la]; A.nt = B.n[ta]; A.n = B.n[dir];
-  // segment length: enough CTAs for ~4 waves of 148 SMs x 2 CTAs, segments of at least 16 points
   const long long lanes = (long long)A.nl * A.nt;
   const long long ctas_per_seg = (lanes + MT - 1) / MT;
-  long long nseg = (148LL * 2 * 4 + ctas_per_seg - 1) / ctas_per_seg;
-  const long long maxseg = A.n / 16 > 0 ? A.n / 16 : 1;
-  if (nseg > maxseg) nseg = maxseg;
-  if (nseg < 1) nseg = 1;
-  A.S = (int)((A.n + nseg - 1) / nseg);
+  const int nseg = pick_segments(ctas_per_seg, A.n);
+  A.S = (A.n + nseg - 1) / nseg;
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;
   if (acc == 0) launch_march_t<0>(c, A, visc);
   else if (acc == 1) launch_march_t<1>(c, A, visc);
   else launch_march_t<2>(c, A, visc);
+  c->launches++;
+  return 0;
+}
+
+// The xi sweep of block B as a staged marching sweep (k_march_xi) with accumulation mode acc.
+int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
+  const bool visc = false;  // the viscous xi derivative comes from k_visc_flux<true> (added by the eta sweep)
+  const long long o0 = B.idx(0, 0, 0);
+  XiArgs A;
+  A.q = B.q + o0;
+  A.kh = B.khat + o0;
+  A.W = visc ? c->ws + o0 : nullptr;
+  A.jac = B.jac + o0;
+  A.r = B.r + o0;
+  A.M = B.M;
+  A.sl = B.s[1]; A.st = B.s[2];
+  A.nl = B.n[1]; A.nt = B.n[2]; A.n = B.n[0];
+  A.nlb = (A.nl + 31) / 32;
+  A.ph = (4 - (NG & 3)) & 3;
+  const long long units = (long long)A.nlb * A.nt;
+  const int nseg = pick_segments((units + XWARPS - 1) / XWARPS, A.n);
+  A.S = (A.n + nseg - 1) / nseg;
+  A.gamma = c->pd.gamma;
+  A.eps4 = 4.0 * c->pd.eps;
+  if (acc == 0) launch_march_xi_t<0>(c, A, visc);
+  else if (acc == 1) launch_march_xi_t<1>(c, A, visc);
+  else launch_march_xi_t<2>(c, A, visc);
   c->launches++;
   return 0;
 }

@@ -30,57 +30,100 @@ __device__ __forceinline__ double d6c(double m3, double m2, double m1, double p1
 // central differences + chain rule (Eq. 21), tau and beta (Eq. 6), then the three directional fluxes (Eq. 5; rows
 // 2..5, row 1 is identically zero) into W[d*4 + (m-1)][M].  Ghost points only get the flux of their own
 // direction (the only one ever differentiated there).
-__global__ void __launch_bounds__(128) k_visc_flux(BlockDev B, ParamsDev P, const double* __restrict__ phi, double* __restrict__ W) {
-  const int e0 = B.n[0] + 6;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x - 3;
+// One CTA = one run of T points along i (plus 3 on either side) at fixed (j, k).  SXI: the xi flux rows stay in
+// shared memory and the CTA writes their 6th-order central xi-derivative S = d(Fv^xi)/d(xi) on interior
+// points instead of the rows themselves (rows W[0..3]); the eta sweep adds S to r (the xi marching sweep then needs
+// no viscous input).  !SXI: the xi rows are written as they are (sweep plans 1-3 differentiate them in the xi sweep).
+template <bool SXI>
+__global__ void __launch_bounds__(256) k_visc_flux(BlockDev B, ParamsDev P, const double* __restrict__ phi, double* __restrict__ W,
+                                                   int T) {
+  __shared__ double sW[4][256];
+  const int i0 = blockIdx.x * T;
+  const int t = threadIdx.x;           // point i = i0 - 3 + t,  t in [0, T + 6)
+  const int i = i0 - 3 + t;
   const int j = blockIdx.y - 3, k = blockIdx.z - 3;
-  if (i >= e0 - 3) return;
+  const int iend = min(i0 + T, B.n[0]);  // SXI: this CTA's outputs are [i0, iend), read with a halo of 3
   const int oi = (i < 0 || i >= B.n[0]), oj = (j < 0 || j >= B.n[1]), ok = (k < 0 || k >= B.n[2]);
-  if (oi + oj + ok > 1) return;
-  const long long M = B.M, p = B.idx(i, j, k);
-  double dphi[3][4];
+  // own: point this CTA writes point-wise results for;  halo: only its xi rows are needed (for the xi derivative)
+  const bool own = SXI ? (i >= i0 && i < iend) : (t < T && i < B.n[0] + 3);
+  const bool halo = SXI && !own && t < (iend - i0) + 6;
+  const bool row_in = (oj + ok) == 0;
+  const bool need_xi = row_in && (own || halo);
+  const bool need_other = own && !oi;
+  const bool work = (need_xi || need_other) && (oi + oj + ok) <= 1 && i >= -3 && i < B.n[0] + 3;
+  const long long M = B.M;
+  if (work) {
+    const long long p = B.idx(i, j, k);
+    double dphi[3][4];
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    const long long st = B.s[d];
+    for (int d = 0; d < 3; ++d) {
+      const long long st = B.s[d];
 #pragma unroll
-    for (int f = 0; f < 4; ++f) {
-      const double* a = phi + f * M + p;
-      dphi[d][f] = d6c(a[-3 * st], a[-2 * st], a[-st], a[st], a[2 * st], a[3 * st]);
+      for (int f = 0; f < 4; ++f) {
+        const double* a = phi + f * M + p;
+        dphi[d][f] = d6c(a[-3 * st], a[-2 * st], a[-st], a[st], a[2 * st], a[3 * st]);
+      }
+    }
+    double kh[3][3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) kh[d][c] = B.khat[(d * 3 + c) * M + p];
+    const double J = B.jac[p];
+    double g[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int f = 0; f < 4; ++f) g[c][f] = J * ((kh[0][c] * dphi[0][f] + kh[1][c] * dphi[1][f]) + kh[2][c] * dphi[2][f]);
+    const double u = phi[p], v = phi[M + p], w = phi[2 * M + p];
+    const double mu = P.mu, kap = P.kappa;
+    const double div = g[0][0] + g[1][1] + g[2][2];
+    const double lam = -(2.0 / 3.0) * mu;
+    const double txx = lam * div + 2.0 * mu * g[0][0];
+    const double tyy = lam * div + 2.0 * mu * g[1][1];
+    const double tzz = lam * div + 2.0 * mu * g[2][2];
+    const double txy = mu * (g[1][0] + g[0][1]);
+    const double txz = mu * (g[2][0] + g[0][2]);
+    const double tyz = mu * (g[2][1] + g[1][2]);
+    const double bx = u * txx + v * txy + w * txz + kap * g[0][3];
+    const double by = u * txy + v * tyy + w * tyz + kap * g[1][3];
+    const double bz = u * txz + v * tyz + w * tzz + kap * g[2][3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      if ((oi && d != 0) || (oj && d != 1) || (ok && d != 2)) continue;
+      const double a = kh[d][0], b = kh[d][1], c = kh[d][2];
+      const double w0 = a * txx + b * txy + c * txz;
+      const double w1 = a * txy + b * tyy + c * tyz;
+      const double w2 = a * txz + b * tyz + c * tzz;
+      const double w3 = a * bx + b * by + c * bz;
+      if (d == 0 && SXI) {
+        sW[0][t] = w0; sW[1][t] = w1; sW[2][t] = w2; sW[3][t] = w3;
+      } else if (own) {
+        W[(d * 4 + 0) * M + p] = w0;
+        W[(d * 4 + 1) * M + p] = w1;
+        W[(d * 4 + 2) * M + p] = w2;
+        W[(d * 4 + 3) * M + p] = w3;
+      }
     }
   }
-  double kh[3][3];
+  if (SXI) {
+    __syncthreads();
+    if (own && row_in && !oi) {
+      const long long p = B.idx(i, j, k);
 #pragma unroll
-  for (int d = 0; d < 3; ++d)
-#pragma unroll
-    for (int c = 0; c < 3; ++c) kh[d][c] = B.khat[(d * 3 + c) * M + p];
-  const double J = B.jac[p];
-  double g[3][4];
-#pragma unroll
-  for (int c = 0; c < 3; ++c)
-#pragma unroll
-    for (int f = 0; f < 4; ++f) g[c][f] = J * ((kh[0][c] * dphi[0][f] + kh[1][c] * dphi[1][f]) + kh[2][c] * dphi[2][f]);
-  const double u = phi[p], v = phi[M + p], w = phi[2 * M + p];
-  const double mu = P.mu, kap = P.kappa;
-  const double div = g[0][0] + g[1][1] + g[2][2];
-  const double lam = -(2.0 / 3.0) * mu;
-  const double txx = lam * div + 2.0 * mu * g[0][0];
-  const double tyy = lam * div + 2.0 * mu * g[1][1];
-  const double tzz = lam * div + 2.0 * mu * g[2][2];
-  const double txy = mu * (g[1][0] + g[0][1]);
-  const double txz = mu * (g[2][0] + g[0][2]);
-  const double tyz = mu * (g[2][1] + g[1][2]);
-  const double bx = u * txx + v * txy + w * txz + kap * g[0][3];
-  const double by = u * txy + v * tyy + w * tyz + kap * g[1][3];
-  const double bz = u * txz + v * tyz + w * tzz + kap * g[2][3];
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    if ((oi && d != 0) || (oj && d != 1) || (ok && d != 2)) continue;
-    const double a = kh[d][0], b = kh[d][1], c = kh[d][2];
-    W[(d * 4 + 0) * M + p] = a * txx + b * txy + c * txz;
-    W[(d * 4 + 1) * M + p] = a * txy + b * tyy + c * tyz;
-    W[(d * 4 + 2) * M + p] = a * txz + b * tyz + c * tzz;
-    W[(d * 4 + 3) * M + p] = a * bx + b * by + c * bz;
+      for (int m = 0; m < 4; ++m)
+        W[(long long)m * M + p] = d6c(sW[m][t - 3], sW[m][t - 2], sW[m][t - 1], sW[m][t + 1], sW[m][t + 2], sW[m][t + 3]);
+    }
   }
+}
+
+// launch geometry of k_visc_flux: runs of T points along i, T + 6 <= 256 threads, all runs equally long
+static void visc_geometry(const BlockDev& B, bool sxi, int* T, dim3* grid, int* threads) {
+  const int span = sxi ? B.n[0] : B.n[0] + 6;  // !SXI: the i-ghost points are "own" points of the first / last run
+  const int nrun = (span + 249) / 250;
+  *T = (span + nrun - 1) / nrun;
+  *threads = ((*T + 6 + 31) / 32) * 32;
+  *grid = dim3(nrun, B.n[1] + 6, B.n[2] + 6);
 }
 
 int launch_rhs(cfd_ctx* c) {
@@ -89,8 +132,15 @@ int launch_rhs(cfd_ctx* c) {
     if (c->pd.viscous) {
       double* phi = c->ws + 12 * c->max_M;
       { ProfScope ps(c, PK_VISC_PHI); k_phi<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, c->pd.gamma, phi); }
-      dim3 g1((B.n[0] + 6 + 127) / 128, B.n[1] + 6, B.n[2] + 6);
-      { ProfScope ps(c, PK_VISC_FLUX); k_visc_flux<<<g1, 128, 0, c->stream>>>(B, c->pd, phi, c->ws); }
+      const bool sxi = c->sweep_plan == 0;
+      int T, threads;
+      dim3 g1;
+      visc_geometry(B, sxi, &T, &g1, &threads);
+      {
+        ProfScope ps(c, PK_VISC_FLUX);
+        if (sxi) k_visc_flux<true><<<g1, threads, 0, c->stream>>>(B, c->pd, phi, c->ws, T);
+        else k_visc_flux<false><<<g1, threads, 0, c->stream>>>(B, c->pd, phi, c->ws, T);
+      }
       c->launches += 2;
     }
     launch_sweeps(c, B);
