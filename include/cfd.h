@@ -126,9 +126,24 @@ int cfd_apply_bc(cfd_ctx*);
 /* Convenience: the four calls above for one stage, in Fig. 2's order, on the context's stream. */
 int cfd_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
 
+/* The same stage with the RK update fused into the last inviscid sweep (default sweep plan; other plans fall back
+ * to cfd_stage): the zeta sweep forms R = J (r + X) point by point and writes a q^n + b (q + dt R) (Eq. 20) straight
+ * into the r buffer, so R is never stored and no separate RK pass runs; stage 1 also reduces res_m = sum R_m^2
+ * (fixed order).  Because q cannot be overwritten while neighbouring points still read it, the three state
+ * buffers of every block EXCHANGE ROLES instead of being copied: after stage 1 the old r buffer holds q, the old
+ * q buffer holds q^n and the old q^n buffer is the scratch r; after stages 2 and 3 q and r swap.
+ * cfd_buffer_roles tells which of the caller's buffers currently plays which role; every other entry point
+ * (cfd_rhs, cfd_rk_stage, cfd_exchange_interfaces, cfd_apply_bc, cfd_step_host) follows the current roles.
+ * The contents of the r buffer after this call are scratch.  res5_host_or_null as in cfd_rk_stage. */
+int cfd_stage_fused(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
+
+/* roles[0], roles[1], roles[2] = which buffer of cfd_block_ptrs (0 = the one passed as q, 1 = qn, 2 = r)
+ * currently holds Q, Q^n and R / scratch.  (0, 1, 2) until cfd_stage_fused or cfd_step_host is used. */
+int cfd_buffer_roles(const cfd_ctx*, int roles[3]);
+
 /* End-to-end entry with HOST buffers (bench.py's e2e leg): for every block b, copies the interior state
  * q_in_host[b] (layout [5][nk][nj][ni], fp64, i fastest, no ghost layers; pinned memory recommended)
- * into the device q, fills ghosts (S6, S5), runs one TVD-RK3 step (three cfd_stage calls, Eq. 20,
+ * into the device q, fills ghosts (S6, S5), runs one TVD-RK3 step (three cfd_stage_fused calls, Eq. 20,
  * P:L173–180), copies the interior of q back into q_out_host[b] (same layout; may alias q_in_host[b])
  * and synchronises the stream.  res5_host_or_null as in cfd_rk_stage.  Returns host values. */
 int cfd_step_host(cfd_ctx*, const double* const* q_in_host, double* const* q_out_host, double dt,

@@ -19,7 +19,7 @@ ABI_SYMBOLS = (
     "cfd_workspace_bytes", "cfd_create_blocks", "cfd_compute_metrics", "cfd_rhs", "cfd_rk_stage",
     "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
-    "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan",
+    "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan", "cfd_stage_fused", "cfd_buffer_roles",
 )
 PROF_NCLASS = 12
 
@@ -62,7 +62,9 @@ def _load():
     for n in ("cfd_compute_metrics", "cfd_rhs", "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_destroy"):
         getattr(L, n).restype = C.c_int
         getattr(L, n).argtypes = [C.c_void_p]
-    for n in ("cfd_rk_stage", "cfd_stage"):
+    L.cfd_buffer_roles.restype = C.c_int
+    L.cfd_buffer_roles.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
+    for n in ("cfd_rk_stage", "cfd_stage", "cfd_stage_fused"):
         getattr(L, n).restype = C.c_int
         getattr(L, n).argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_double)]
     L.cfd_last_error.restype = C.c_char_p
@@ -173,8 +175,20 @@ class Context:
             raise CfdError(rc, lib.cfd_last_error(self.h).decode())
 
     # ---- data movement helpers (harness side) ----
+    def buffer_roles(self):
+        """cfd_buffer_roles: which of the buffers allocated as (q, qn, r) currently holds Q, Q^n, R."""
+        r = (C.c_int * 3)()
+        self._chk(lib.cfd_buffer_roles(self.h, r))
+        return tuple(r[:])
+
+    def field(self, b, name):
+        """The tensor that currently plays the role `name` (cfd_stage_fused exchanges the roles of q, qn, r)."""
+        if name in ("q", "qn", "r"):
+            name = ("q", "qn", "r")[self.buffer_roles()[("q", "qn", "r").index(name)]]
+        return self.fields[b][name]
+
     def interior(self, b, name):
-        return self.fields[b][name][:, NG:-NG, NG:-NG, NG:-NG]
+        return self.field(b, name)[:, NG:-NG, NG:-NG, NG:-NG]
 
     def load_case(self, case):
         t = self.torch
@@ -186,7 +200,7 @@ class Context:
         self.apply_bc()
 
     def to_numpy(self, b, name, interior=True):
-        a = self.interior(b, name) if interior else self.fields[b][name]
+        a = self.interior(b, name) if interior else self.field(b, name)
         return a.detach().cpu().numpy()
 
     # ---- the C ABI, same names ----
@@ -212,11 +226,17 @@ class Context:
         self._chk(lib.cfd_stage(self.h, int(stage), float(dt), res if want_res else None))
         return np.array(res[:]) if want_res else None
 
-    def step(self, dt, want_res=False):
-        """One TVD-RK3 step = three stages in the order of Fig. 2."""
+    def stage_fused(self, stage, dt, want_res=False):
+        res = (C.c_double * 5)()
+        self._chk(lib.cfd_stage_fused(self.h, int(stage), float(dt), res if want_res else None))
+        return np.array(res[:]) if want_res else None
+
+    def step(self, dt, want_res=False, fused=True):
+        """One TVD-RK3 step = three stages in the order of Fig. 2; fused: cfd_stage_fused (the RK update
+        inside the last sweep, buffer roles exchanged) instead of cfd_stage."""
         res = None
         for s in (1, 2, 3):
-            r = self.stage(s, dt, want_res=(want_res and s == 1))
+            r = (self.stage_fused if fused else self.stage)(s, dt, want_res=(want_res and s == 1))
             if s == 1:
                 res = r
         return res

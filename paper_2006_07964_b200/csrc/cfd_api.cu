@@ -10,7 +10,7 @@ static thread_local std::string g_create_err;
 static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD_FACE_INTERFACE; }
 
 size_t ws_partials_offset_doubles(long long max_M) { return (size_t)16 * (size_t)max_M; }
-int rk_max_partial_blocks() { return 4096; }
+int rk_max_partial_blocks() { return 16384; }
 
 extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
   long long mx = 0;
@@ -19,6 +19,24 @@ extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const c
     if (M > mx) mx = M;
   }
   return (ws_partials_offset_doubles(mx) + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
+}
+
+// the six assignments of three buffers to the roles (q, qn, r): id -> role[]
+static void roles_of(int id, int r[3]) {
+  static const int P[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+  for (int x = 0; x < 3; ++x) r[x] = P[id][x];
+}
+void set_roles(cfd_ctx* c, int iq, int iqn, int ir) {
+  c->role[0] = iq; c->role[1] = iqn; c->role[2] = ir;
+  int id = 0;
+  for (; id < 6; ++id) {
+    int r[3];
+    roles_of(id, r);
+    if (r[0] == iq && r[1] == iqn && r[2] == ir) break;
+  }
+  const size_t nb = c->blk.size();
+  for (size_t b = 0; b < nb; ++b) { c->blk[b].q = c->base[iq][b]; c->blk[b].qn = c->base[iqn][b]; c->blk[b].r = c->base[ir][b]; }
+  c->d_blocks = c->d_blocks_all + (size_t)id * nb;
 }
 
 static int fail_create(int code, const std::string& msg) {
@@ -165,8 +183,24 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
     return fail_create(CFD_E_CUDA, m);
   };
   cudaError_t e;
-  if ((e = cudaMalloc(&c->d_blocks, sizeof(BlockDev) * nblocks)) != cudaSuccess) return cuda_fail(e, "cudaMalloc blocks");
-  if ((e = cudaMemcpy(c->d_blocks, c->blk.data(), sizeof(BlockDev) * nblocks, cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy blocks");
+  // one descriptor array per assignment of the caller's (q, qn, r) buffers to the three roles: the fused stage
+  // (cfd_stage_fused) exchanges roles instead of copying
+  for (int b = 0; b < nblocks; ++b) { c->base[0].push_back(ptrs[b].q); c->base[1].push_back(ptrs[b].qn); c->base[2].push_back(ptrs[b].r); }
+  if ((e = cudaMalloc(&c->d_blocks_all, sizeof(BlockDev) * nblocks * 6)) != cudaSuccess) return cuda_fail(e, "cudaMalloc blocks");
+  {
+    std::vector<BlockDev> all((size_t)nblocks * 6);
+    for (int id = 0; id < 6; ++id) {
+      int r[3];
+      roles_of(id, r);
+      for (int b = 0; b < nblocks; ++b) {
+        BlockDev B = c->blk[b];
+        B.q = c->base[r[0]][b]; B.qn = c->base[r[1]][b]; B.r = c->base[r[2]][b];
+        all[(size_t)id * nblocks + b] = B;
+      }
+    }
+    if ((e = cudaMemcpy(c->d_blocks_all, all.data(), sizeof(BlockDev) * all.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy blocks");
+  }
+  set_roles(c, 0, 1, 2);
   for (int p = 1; p <= 3; ++p) {
     if (c->tasks[p].empty()) continue;
     if ((e = cudaMalloc(&c->d_tasks[p], sizeof(CopyTask) * c->tasks[p].size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc tasks");
@@ -182,7 +216,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
 
 extern "C" int cfd_destroy(cfd_ctx* c) {
   if (!c) return CFD_OK;
-  if (c->d_blocks) cudaFree(c->d_blocks);
+  if (c->d_blocks_all) cudaFree(c->d_blocks_all);
   for (int p = 1; p <= 3; ++p)
     if (c->d_tasks[p]) cudaFree(c->d_tasks[p]);
   if (c->d_flag) cudaFree(c->d_flag);
@@ -211,7 +245,7 @@ extern "C" int cfd_compute_metrics(cfd_ctx* c) {
 
 extern "C" int cfd_rhs(cfd_ctx* c) {
   if (!c) return CFD_E_ARG;
-  return launch_rhs(c);
+  return launch_rhs(c, 0, 0.0);
 }
 
 extern "C" int cfd_rk_stage(cfd_ctx* c, int stage, double dt, double* res5) {
@@ -244,6 +278,29 @@ extern "C" int cfd_stage(cfd_ctx* c, int stage, double dt, double* res5) {
   return cfd_apply_bc(c);
 }
 
+extern "C" int cfd_stage_fused(cfd_ctx* c, int stage, double dt, double* res5) {
+  if (!c) return CFD_E_ARG;
+  if (stage < 1 || stage > 3) { c->err = "cfd_stage_fused: stage must be 1..3"; return CFD_E_STAGE; }
+  if (c->sweep_plan != 0) return cfd_stage(c, stage, dt, res5);  // only the default plan has the fused last sweep
+  int rc = launch_rhs(c, stage, dt);
+  if (rc != 0) return rc;
+  // the new state was written to the r buffers: exchange the roles (stage 1: the old q becomes q^n, Eq. 20)
+  if (stage == 1) set_roles(c, c->role[2], c->role[0], c->role[1]);
+  else set_roles(c, c->role[2], c->role[1], c->role[0]);
+  if (res5 && stage == 1) {
+    CUDA_TRY(c, cudaMemcpyAsync(res5, c->d_res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  }
+  if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
+  return cfd_apply_bc(c);
+}
+
+extern "C" int cfd_buffer_roles(const cfd_ctx* c, int roles[3]) {
+  if (!c || !roles) return CFD_E_ARG;
+  for (int x = 0; x < 3; ++x) roles[x] = c->role[x];
+  return CFD_OK;
+}
+
 extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const* qout, double dt, double* res5) {
   if (!c || !qin || !qout) return CFD_E_ARG;
   auto copy3d = [&](const BlockDev& B, double* dev, double* host, bool to_dev) {
@@ -269,7 +326,7 @@ extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const
   if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
   if ((rc = cfd_apply_bc(c)) != 0) return rc;
   for (int s = 1; s <= 3; ++s)
-    if ((rc = cfd_stage(c, s, dt, nullptr)) != 0) return rc;
+    if ((rc = cfd_stage_fused(c, s, dt, nullptr)) != 0) return rc;
   for (size_t b = 0; b < c->blk.size(); ++b) {
     const BlockDev& B = c->blk[b];
     const size_t N = (size_t)B.n[0] * B.n[1] * B.n[2];

@@ -53,7 +53,10 @@ struct cfd_ctx {
   std::vector<CopyTask> tasks[4];     // per pass 1..3
   std::vector<BcTask> bcs;
   CopyTask* d_tasks[4] = {nullptr, nullptr, nullptr, nullptr};
-  BlockDev* d_blocks = nullptr;
+  BlockDev* d_blocks = nullptr;       // the descriptor array of the current buffer roles (points into d_blocks_all)
+  BlockDev* d_blocks_all = nullptr;   // [6][nblocks]: one array per assignment of the three state buffers to (q, qn, r)
+  std::vector<double*> base[3];       // per block: the caller's q, qn, r buffers as given to cfd_create_blocks
+  int role[3] = {0, 1, 2};            // role[x] = which base buffer currently serves as q (x=0), qn (1), r (2)
   int* d_flag = nullptr;              // J <= 0 flag
   double* d_res = nullptr;            // 5 residual sums
   cudaStream_t stream = nullptr;
@@ -96,12 +99,21 @@ struct ProfScope {
   }
 };
 
+// RK stage fused into the last marching sweep (k_march ACC 3)
+struct RkFuse {
+  int stage;          // 1..3
+  double dt, a, b;    // Eq. 20: out = a q^n + b (q + dt R)
+  double* partials;   // stage 1: where this launch writes its per-CTA partial sums of R_m^2 (5 per CTA)
+  long long max_ctas; // capacity of partials / 5
+};
+
 // ---- kernel launchers (each enqueues on ctx->stream and bumps ctx->launches) --------------------
 int launch_fill_connect(cfd_ctx* c, int field /*0 q, 1 xyz*/);
 int launch_bc_xyz(cfd_ctx* c);
 int launch_bc_q(cfd_ctx* c);
 int launch_metrics(cfd_ctx* c);
-int launch_rhs(cfd_ctx* c);
+int launch_rhs(cfd_ctx* c, int fused_stage /*0 = plain rhs*/, double dt);
+void set_roles(cfd_ctx* c, int iq, int iqn, int ir);
 int launch_rk(cfd_ctx* c, int stage, double dt);
 int launch_fp64_probe(int iters, double* tflops);
 int launch_fastmath_selftest(int n, const double* x_host, double* rcp_host, double* rsqrt_host);

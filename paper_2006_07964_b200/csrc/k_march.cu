@@ -32,12 +32,14 @@ struct MarchArgs {
   const double* kh;     // khat^d, + interior origin
   const double* W;      // viscous flux rows of direction d, + interior origin (VISC)
   const double* jac;    // + interior origin (ACC 2)
-  const double* Sx;     // d(Fv^xi)/d(xi) rows from k_visc_flux<true>, + interior origin, or null (added to r when ACC >= 1)
+  const double* qn;     // q^n + interior origin (ACC 3, stages 2 and 3)
   double* r;            // + interior origin
+  double* partials;     // ACC 3 stage 1: 5 partial sums of R_m^2 per CTA
   long long M;          // plane stride between variables
   long long sl, sm, st; // strides: neighbouring lane, one step along the sweep, third index
   int nl, nt, n, S;     // lanes, third extent, sweep length, segment length
   double gamma, eps4;
+  double dt, rk_a, rk_b; // ACC 3 (Eq. 20)
 };
 
 __device__ __forceinline__ void cp8(double* dst, const double* src) {
@@ -76,135 +78,195 @@ __device__ __forceinline__ double fir_push2(double acc[5], double x, double xv) 
   return out;
 }
 
-// ACC 0: r = X;  1: r += X;  2: r = J (r + X)   with X = dFv/dxi^d - D^d = -(Phi_{j+1/2} - Phi_{j-1/2})
-template <int ACC, bool VISC, bool SX>
-__global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
-  extern __shared__ double ring[];  // [RING][RV][MT], thread-private columns
-  const int tid = threadIdx.x;
-  const long long L = (long long)blockIdx.x * MT + tid;
-  if (L >= (long long)A.nl * A.nt) return;  // no barriers in this kernel
-  const int il = (int)(L % A.nl), it = (int)(L / A.nl);
-  const int p0 = blockIdx.y * A.S;
-  const int p1 = min(A.n, p0 + A.S);
-  const long long base = il * A.sl + it * A.st;
-  const double* __restrict__ q = A.q + base;
-  const double* __restrict__ kh = A.kh + base;
-  const double* __restrict__ W = VISC ? A.W + base : nullptr;
-  double* __restrict__ r = A.r + base;
-  const long long M = A.M, sm = A.sm;
-  const double gamma = A.gamma, eps4 = A.eps4;
-  double* const col = ring + tid;
-#define SLOT(p) (col + (((p) + 8) & 7) * (RV * MT))
-  auto fetch = [&](int p) {
-    double* s = SLOT(p);
-    const long long o = p * sm;
-#pragma unroll
-    for (int m = 0; m < 5; ++m) cp8(s + m * MT, q + m * M + o);
-#pragma unroll
-    for (int c = 0; c < 3; ++c) cp8(s + (5 + c) * MT, kh + c * M + o);
-  };
-  // ---- prologue: positions p0-4 .. p0+1 (first step j = p0-1 reads Q j-2..j+2 and khat j-3..j+2) ----
-  for (int p = p0 - 4; p <= p0 + 1; ++p) fetch(p);
-  cp_commit();
-  double acc[5][5];
-#pragma unroll
-  for (int m = 0; m < 5; ++m)
-#pragma unroll
-    for (int t = 0; t < 5; ++t) acc[m][t] = 0.0;
-  cp_wait<0>();
-  // prime the FIR with the point fluxes of p0-3 .. p0 (the loop then pushes F_{j+2} at step j)
-  for (int p = p0 - 3; p <= p0; ++p) {
-    const double* s = SLOT(p);
-    double F[5];
-    point_flux(s[0], s[MT], s[2 * MT], s[3 * MT], s[4 * MT], s[5 * MT], s[6 * MT], s[7 * MT], gamma, F);
-    fir_push(acc[0], F[0]);
-#pragma unroll
-    for (int m = 1; m < 5; ++m) {
-      if (VISC) fir_push2(acc[m], F[m], W[(long long)(m - 1) * M + p * sm]);
-      else fir_push(acc[m], F[m]);
-    }
-  }
-  double ULc[5] = {0, 0, 0, 0, 0}, Phip[5] = {0, 0, 0, 0, 0};
-  double wv[4] = {0, 0, 0, 0};
-  if (VISC) {
-#pragma unroll
-    for (int m = 0; m < 4; ++m) wv[m] = W[(long long)m * M + (p0 + 1) * sm];
-  }
-  for (int j = p0 - 1; j <= p1; ++j) {
-    // ---- prefetch position j+3 for the next step ----
-    if (j < p1) fetch(j + 3);
-    cp_commit();
-    double wn[4] = {0, 0, 0, 0};
-    if (VISC && j < p1) {
-#pragma unroll
-      for (int m = 0; m < 4; ++m) wn[m] = W[(long long)m * M + (long long)(j + 3) * sm];
-    }
-    double rold[5] = {0, 0, 0, 0, 0}, jac = 0.0;
-    if (ACC >= 1 && j > p0) {
-#pragma unroll
-      for (int m = 0; m < 5; ++m) rold[m] = r[m * M + (long long)(j - 1) * sm];
-      if (SX) {
-#pragma unroll
-        for (int m = 1; m < 5; ++m) rold[m] += A.Sx[base + (long long)(m - 1) * M + (long long)(j - 1) * sm];
-      }
-      if (ACC == 2) jac = A.jac[base + (long long)(j - 1) * sm];
-    }
-    cp_wait<1>();
-    // ---- point j: U^L_{j+1/2}, U^R_{j-1/2} ----
-    double Qs[5][5], UL[5], UR[5], Fc[5];
-#pragma unroll
-    for (int s = 0; s < 5; ++s) {
-      const double* sl = SLOT(j - 2 + s);
-#pragma unroll
-      for (int m = 0; m < 5; ++m) Qs[s][m] = sl[m * MT];
-    }
-    const double* sc = SLOT(j);
-    afweno_states(Qs, sc[5 * MT], sc[6 * MT], sc[7 * MT], gamma, eps4, UL, UR, Fc);
-    // ---- FIR: push the point flux of j+2; output = central + viscous part of Phi_{j-1/2} ----
-    double G[5];
-    {
-      const double* s2 = SLOT(j + 2);
-      double F[5];
-      point_flux(Qs[4][0], Qs[4][1], Qs[4][2], Qs[4][3], Qs[4][4], s2[5 * MT], s2[6 * MT], s2[7 * MT], gamma, F);
-      G[0] = fir_push(acc[0], F[0]);
-#pragma unroll
-      for (int m = 1; m < 5; ++m) G[m] = VISC ? fir_push2(acc[m], F[m], wv[m - 1]) : fir_push(acc[m], F[m]);
-    }
-    if (j >= p0) {
-      // ---- interface j-1/2: metric (U5), both split fluxes, numerical flux ----
-      const double *k0 = SLOT(j - 3), *k1 = SLOT(j - 2), *k2 = SLOT(j - 1), *k4 = SLOT(j + 1), *k5 = SLOT(j + 2);
-      const double kx = khalf(k0[5 * MT], k1[5 * MT], k2[5 * MT], sc[5 * MT], k4[5 * MT], k5[5 * MT]);
-      const double ky = khalf(k0[6 * MT], k1[6 * MT], k2[6 * MT], sc[6 * MT], k4[6 * MT], k5[6 * MT]);
-      const double kz = khalf(k0[7 * MT], k1[7 * MT], k2[7 * MT], sc[7 * MT], k4[7 * MT], k5[7 * MT]);
-      const double kk = fma(kx, kx, fma(ky, ky, kz * kz));
-      const double ikn = frsqrt(kk), kn = kk * ikn;
-      double Fp[5], Fm[5];
-      sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
-      sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
-#pragma unroll
-      for (int m = 0; m < 5; ++m) {
-        const double Phi = (Fp[m] + Fm[m]) + G[m];
-        if (j > p0) {
-          const double X = Phip[m] - Phi;
-          double* rp = r + m * M + (long long)(j - 1) * sm;
-          if (ACC == 0) *rp = X;
-          else if (ACC == 1) *rp = rold[m] + X;
-          else *rp = jac * (rold[m] + X);
-        }
-        Phip[m] = Phi;
-      }
-    }
-#pragma unroll
-    for (int m = 0; m < 5; ++m) ULc[m] = UL[m];
-    if (VISC) {
-#pragma unroll
-      for (int m = 0; m < 4; ++m) wv[m] = wn[m];
-    }
-  }
-#undef SLOT
+// ACC 0: r = X;  1: r += X;  2: r = J (r + X);  3: the RK stage fused into the last sweep (Eq. 20):
+//   with R = J (r + X):  out = a q^n + b (q + dt R)  written to the r buffer (the caller then exchanges the roles of the
+//   q and r buffers; q itself cannot be overwritten while neighbouring threads still read it).  ST1 (stage 1):
+//   a = 0, b = 1, q^n is not read (the old q buffer becomes q^n by the same exchange) and the CTA writes its
+//   partial sums of R_m^2 (U17; fixed order: run-to-run deterministic).
+//   X = dFv/dxi^d - D^d = -(Phi_{j+1/2} - Phi_{j-1/2}).
+// Every operand arrives through thread-private shared-memory columns filled by cp.async one step ahead (Q, khat of
+// position j+3; the viscous rows of j+3; old r, J, q^n of the output position): nothing is held in registers across
+// a step, which is what the register allocation of this kernel (~250 registers, 2 CTAs per SM) needs.
+template <int ACC, bool ST1>
+struct OutCfg {
+  static constexpr int O_R = 0;                                  // old r (5), ACC >= 1
+  static constexpr int O_J = ACC >= 1 ? 5 : 0;                   // J (1), ACC >= 2
+  static constexpr int O_QN = O_J + (ACC >= 2 ? 1 : 0);          // q^n (5), ACC 3 stages 2, 3
+  static constexpr int NOUT = O_QN + ((ACC == 3 && !ST1) ? 5 : 0);
+};
+template <int ACC, bool VISC, bool ST1>
+constexpr int march_smem_doubles() {
+  return (RING * RV + (VISC ? 8 : 0) + 2 * OutCfg<ACC, ST1>::NOUT + ((ACC == 3 && ST1) ? 5 : 0)) * MT;
 }
 
-
+template <int ACC, bool VISC, bool ST1>
+__global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
+  extern __shared__ double ring[];  // thread-private columns: [RING][RV][MT] | W [2][4][MT] | out operands [2][NOUT][MT] | res [5][MT]
+  using OC = OutCfg<ACC, ST1>;
+  constexpr int NOUT = OC::NOUT;
+  const int tid = threadIdx.x;
+  const long long L = (long long)blockIdx.x * MT + tid;
+  const bool live = L < (long long)A.nl * A.nt;
+  double* const col = ring + tid;
+  double* const wcol = col + RING * RV * MT;
+  double* const ocol = wcol + (VISC ? 8 : 0) * MT;
+  double* const rcol = ocol + 2 * NOUT * MT;
+  if (ACC == 3 && ST1) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) rcol[m * MT] = 0.0;
+  }
+  if (live) {
+    const int il = (int)(L % A.nl), it = (int)(L / A.nl);
+    const int p0 = blockIdx.y * A.S;
+    const int p1 = min(A.n, p0 + A.S);
+    const long long base = il * A.sl + it * A.st;
+    const double* __restrict__ q = A.q + base;
+    const double* __restrict__ kh = A.kh + base;
+    const double* __restrict__ W = VISC ? A.W + base : nullptr;
+    double* __restrict__ r = A.r + base;
+    const long long M = A.M, sm = A.sm;
+    const double gamma = A.gamma, eps4 = A.eps4;
+#define SLOT(p) (col + (((p) + 8) & 7) * (RV * MT))
+    auto fetch = [&](int p) {
+      double* s = SLOT(p);
+      const long long o = p * sm;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) cp8(s + m * MT, q + m * M + o);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) cp8(s + (5 + c) * MT, kh + c * M + o);
+    };
+    auto fetch_w = [&](int p) {
+      double* s = wcol + (p & 1) * (4 * MT);
+      const long long o = p * sm;
+#pragma unroll
+      for (int m = 0; m < 4; ++m) cp8(s + m * MT, W + m * M + o);
+    };
+    auto fetch_out = [&](int p) {  // operands of the output at position p
+      double* s = ocol + (p & 1) * (NOUT * MT);
+      const long long o = p * sm;
+      if (ACC >= 1) {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) cp8(s + (OC::O_R + m) * MT, r + m * M + o);
+      }
+      if (ACC >= 2) cp8(s + OC::O_J * MT, A.jac + base + o);
+      if (ACC == 3 && !ST1) {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) cp8(s + (OC::O_QN + m) * MT, A.qn + base + m * M + o);
+      }
+    };
+    // ---- prologue: positions p0-4 .. p0+1 (first step j = p0-1 reads Q j-2..j+2 and khat j-3..j+2) ----
+    for (int p = p0 - 4; p <= p0 + 1; ++p) fetch(p);
+    if (VISC) fetch_w(p0 + 1);
+    cp_commit();
+    double acc[5][5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m)
+#pragma unroll
+      for (int t = 0; t < 5; ++t) acc[m][t] = 0.0;
+    cp_wait<0>();
+    // prime the FIR with the point fluxes of p0-3 .. p0 (the loop then pushes F_{j+2} at step j)
+    for (int p = p0 - 3; p <= p0; ++p) {
+      const double* s = SLOT(p);
+      double F[5];
+      point_flux(s[0], s[MT], s[2 * MT], s[3 * MT], s[4 * MT], s[5 * MT], s[6 * MT], s[7 * MT], gamma, F);
+      fir_push(acc[0], F[0]);
+#pragma unroll
+      for (int m = 1; m < 5; ++m) {
+        if (VISC) fir_push2(acc[m], F[m], W[(long long)(m - 1) * M + p * sm]);
+        else fir_push(acc[m], F[m]);
+      }
+    }
+    double ULc[5] = {0, 0, 0, 0, 0}, Phip[5] = {0, 0, 0, 0, 0};
+    for (int j = p0 - 1; j <= p1; ++j) {
+      // ---- prefetch for the next step: Q, khat, W of position j+3; operands of the output at position j ----
+      if (j < p1) {
+        fetch(j + 3);
+        if (VISC) fetch_w(j + 3);
+        if (NOUT > 0 && j >= p0) fetch_out(j);
+      }
+      cp_commit();
+      cp_wait<1>();
+      // ---- point j: U^L_{j+1/2}, U^R_{j-1/2} ----
+      double Qs[5][5], UL[5], UR[5], Fc[5];
+#pragma unroll
+      for (int s = 0; s < 5; ++s) {
+        const double* sl = SLOT(j - 2 + s);
+#pragma unroll
+        for (int m = 0; m < 5; ++m) Qs[s][m] = sl[m * MT];
+      }
+      const double* sc = SLOT(j);
+      afweno_states(Qs, sc[5 * MT], sc[6 * MT], sc[7 * MT], gamma, eps4, UL, UR, Fc);
+      // ---- FIR: push the point flux of j+2; output = central + viscous part of Phi_{j-1/2} ----
+      double G[5];
+      {
+        const double* s2 = SLOT(j + 2);
+        const double* sw = wcol + ((j + 2) & 1) * (4 * MT);
+        double F[5];
+        point_flux(Qs[4][0], Qs[4][1], Qs[4][2], Qs[4][3], Qs[4][4], s2[5 * MT], s2[6 * MT], s2[7 * MT], gamma, F);
+        G[0] = fir_push(acc[0], F[0]);
+#pragma unroll
+        for (int m = 1; m < 5; ++m) G[m] = VISC ? fir_push2(acc[m], F[m], sw[(m - 1) * MT]) : fir_push(acc[m], F[m]);
+      }
+      if (j >= p0) {
+        // ---- interface j-1/2: metric (U5), both split fluxes, numerical flux ----
+        const double *k0 = SLOT(j - 3), *k1 = SLOT(j - 2), *k2 = SLOT(j - 1), *k4 = SLOT(j + 1), *k5 = SLOT(j + 2);
+        const double kx = khalf(k0[5 * MT], k1[5 * MT], k2[5 * MT], sc[5 * MT], k4[5 * MT], k5[5 * MT]);
+        const double ky = khalf(k0[6 * MT], k1[6 * MT], k2[6 * MT], sc[6 * MT], k4[6 * MT], k5[6 * MT]);
+        const double kz = khalf(k0[7 * MT], k1[7 * MT], k2[7 * MT], sc[7 * MT], k4[7 * MT], k5[7 * MT]);
+        const double kk = fma(kx, kx, fma(ky, ky, kz * kz));
+        const double ikn = frsqrt(kk), kn = kk * ikn;
+        double Fp[5], Fm[5];
+        sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
+        sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+        const double* so = ocol + ((j - 1) & 1) * (NOUT * MT);
+        double jac = 0.0;
+        if (ACC >= 2 && j > p0) jac = so[OC::O_J * MT];
+#pragma unroll
+        for (int m = 0; m < 5; ++m) {
+          const double Phi = (Fp[m] + Fm[m]) + G[m];
+          if (j > p0) {
+            const double X = Phip[m] - Phi;
+            double* rp = r + m * M + (long long)(j - 1) * sm;
+            if (ACC == 0) *rp = X;
+            else if (ACC == 1) *rp = so[(OC::O_R + m) * MT] + X;
+            else if (ACC == 2) *rp = jac * (so[(OC::O_R + m) * MT] + X);
+            else {
+              const double R = jac * (so[(OC::O_R + m) * MT] + X);
+              const double qc = k2[m * MT];  // Q_m at position j-1
+              if (ST1) {
+                rcol[m * MT] += R * R;
+                *rp = qc + A.dt * R;
+              } else {
+                *rp = A.rk_a * so[(OC::O_QN + m) * MT] + A.rk_b * (qc + A.dt * R);
+              }
+            }
+          }
+          Phip[m] = Phi;
+        }
+      }
+#pragma unroll
+      for (int m = 0; m < 5; ++m) ULc[m] = UL[m];
+    }
+#undef SLOT
+  }
+  if (ACC == 3 && ST1) {
+    // fixed-order partial sums of R_m^2 over this CTA's points
+    __shared__ double swr[5][MT / 32];
+    const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      double v = rcol[m * MT];
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+      if (lane == 0) swr[m][wid] = v;
+    }
+    __syncthreads();
+    if (tid < 5) {
+      double v = 0.0;
+      for (int w = 0; w < MT / 32; ++w) v += swr[tid][w];
+      A.partials[((long long)blockIdx.y * gridDim.x + blockIdx.x) * 5 + tid] = v;
+    }
+  }
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // The xi sweep as a marching sweep with WARP-PRIVATE TRANSPOSED STAGING.  Marching along i puts the lanes of a warp
@@ -218,14 +280,15 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
 // The output of step j (r at position j-1) is parked in the Q slots of position j-3 (dead: Q is read at j-2..j+2 only)
 // and written out by the same lane mapping as the loads, four positions = one full sector per line at a time, just
 // before those slots are refilled; the flush applies the accumulation mode (r = X, r += X, r = J (r + X)).
-constexpr int XR = 10, XW = 5;
-constexpr int XLS = 8 * XR + 4 * XW + 1;  // 101 doubles per line
+constexpr int XR = 10;
+constexpr int XLS = 8 * XR + 1;  // 81 doubles per line
 constexpr int XWARPS = 4;
 
 struct XiArgs {
   const double* q;      // + interior origin
   const double* kh;
-  const double* W;
+  const double* W;      // unused (the viscous xi rows never reach this kernel)
+  const double* Sx;     // VISC: S = d(Fv^xi)/d(xi) rows 2..5 from k_visc_flux<true>, added to r in the flush
   const double* jac;
   double* r;
   long long M;          // plane stride between variables
@@ -265,7 +328,7 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
     goff[t] = tbase + (long long)min(ln, A.nl - 1) * A.sl;
   }
   double* const lbase = wbase + lsub * XLS;  // + t * 8 * XLS
-  const int qlo = p0 - 4, qhi = p1 + 2, wlo = p0 + 1;
+  const int qlo = p0 - 4, qhi = p1 + 2;
 
   auto load_chunk = [&](int c) {
     const int pos = c + lpos;
@@ -280,16 +343,6 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
         for (int m = 0; m < 5; ++m) cp8(d + m * XR, gq + m * M);
 #pragma unroll
         for (int cc = 0; cc < 3; ++cc) cp8(d + (5 + cc) * XR, gk + cc * M);
-      }
-      if (VISC && pos >= wlo) {
-        const int s5 = (pos + 2 * XW) % XW;
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          double* d = lbase + t * 8 * XLS + 8 * XR + s5;
-          const double* gw = A.W + goff[t] + pos;
-#pragma unroll
-          for (int m = 0; m < 4; ++m) cp8(d + m * XW, gw + m * M);
-        }
       }
     }
   };
@@ -307,7 +360,8 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
         if (ACC == 2) jac = A.jac[goff[t] + pos];
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
-          const double X = sX[m * XR];
+          double X = sX[m * XR];
+          if (VISC && m > 0) X += A.Sx[goff[t] + pos + (long long)(m - 1) * M];
           if (ACC == 0) gr[m * M] = X;
           else if (ACC == 1) gr[m * M] = gr[m * M] + X;
           else gr[m * M] = jac * (gr[m * M] + X);
@@ -328,18 +382,9 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
   for (int m = 0; m < 5; ++m)
 #pragma unroll
     for (int t = 0; t < 5; ++t) acc[m][t] = 0.0;
-  const long long myoff = tbase + (long long)min(l0 + lane, A.nl - 1) * A.sl;
-  double wpro[4][4];
-  if (VISC) {  // the four viscous rows that prime the FIR: read directly (once per segment)
-#pragma unroll
-    for (int t = 0; t < 4; ++t)
-#pragma unroll
-      for (int m = 0; m < 4; ++m) wpro[t][m] = A.W[myoff + (long long)m * M + (p0 - 3 + t)];
-  }
   cp_wait<0>();
   __syncwarp();
   int s0 = (p0 - 1 - 3 + 2 * XR) % XR;  // slot of position j-3 at the first step j = p0-1
-  int w5 = (p0 - 1 + 2 + 2 * XW) % XW;  // slot of W at position j+2
   // prime the FIR with the point fluxes of p0-3 .. p0 (slots s0+1 .. s0+4)
 #pragma unroll
   for (int t = 0; t < 4; ++t) {
@@ -348,10 +393,7 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
     point_flux(s[0], s[XR], s[2 * XR], s[3 * XR], s[4 * XR], s[5 * XR], s[6 * XR], s[7 * XR], gamma, F);
     fir_push(acc[0], F[0]);
 #pragma unroll
-    for (int m = 1; m < 5; ++m) {
-      if (VISC) fir_push2(acc[m], F[m], wpro[t][m - 1]);
-      else fir_push(acc[m], F[m]);
-    }
+    for (int m = 1; m < 5; ++m) fir_push(acc[m], F[m]);
   }
   double ULc[5] = {0, 0, 0, 0, 0}, Phip[5] = {0, 0, 0, 0, 0};
   for (int j = p0 - 1; j <= p1; ++j) {
@@ -383,9 +425,8 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
       double F[5];
       point_flux(Qs[4][0], Qs[4][1], Qs[4][2], Qs[4][3], Qs[4][4], sl5[5 * XR], sl5[6 * XR], sl5[7 * XR], gamma, F);
       G[0] = fir_push(acc[0], F[0]);
-      const double* sw = my + 8 * XR + w5;
 #pragma unroll
-      for (int m = 1; m < 5; ++m) G[m] = VISC ? fir_push2(acc[m], F[m], sw[(m - 1) * XW]) : fir_push(acc[m], F[m]);
+      for (int m = 1; m < 5; ++m) G[m] = fir_push(acc[m], F[m]);
     }
     if (j >= p0) {
       // ---- interface j-1/2: metric (U5), both split fluxes, numerical flux ----
@@ -408,7 +449,6 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
 #pragma unroll
     for (int m = 0; m < 5; ++m) ULc[m] = UL[m];
     s0 = wrap10(s0 + 1);
-    w5 = w5 + 1 >= XW ? 0 : w5 + 1;
   }
   // ---- flush what is still parked: groups after the last one flushed in the loop ----
   __syncwarp();
@@ -446,26 +486,28 @@ int pick_segments(long long ctas_per_seg, int n) {
   return best;
 }
 
-template <int ACC>
-void launch_march_t(cfd_ctx* c, const MarchArgs& A, bool visc) {
+template <int ACC, bool VISC, bool ST1>
+void launch_march_k(cfd_ctx* c, const MarchArgs& A) {
   const long long lanes = (long long)A.nl * A.nt;
   dim3 grid((unsigned)((lanes + MT - 1) / MT), (unsigned)((A.n + A.S - 1) / A.S));
-  const size_t smem = sizeof(double) * RING * RV * MT;
-  if (visc && A.Sx != nullptr && ACC == 1) k_march<1, true, true><<<grid, MT, smem, c->stream>>>(A);
-  else if (visc) k_march<ACC, true, false><<<grid, MT, smem, c->stream>>>(A);
-  else k_march<ACC, false, false><<<grid, MT, smem, c->stream>>>(A);
+  const size_t smem = sizeof(double) * march_smem_doubles<ACC, VISC, ST1>();
+  k_march<ACC, VISC, ST1><<<grid, MT, smem, c->stream>>>(A);
+}
+
+template <int ACC, bool VISC, bool ST1>
+cudaError_t march_attr() {
+  return cudaFuncSetAttribute(k_march<ACC, VISC, ST1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)(sizeof(double) * march_smem_doubles<ACC, VISC, ST1>()));
 }
 
 }  // namespace
 
 int march_init() {
   cudaError_t e = cudaSuccess;
-  const int smem = (int)(sizeof(double) * RING * RV * MT);
-#define OPT(A)                                                                                                      \
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<A, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); \
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<A, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-  OPT(0) OPT(1) OPT(2)
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+#define OPT(A, S)                                          \
+  if (e == cudaSuccess) e = march_attr<A, true, S>();      \
+  if (e == cudaSuccess) e = march_attr<A, false, S>();
+  OPT(0, false) OPT(1, false) OPT(2, false) OPT(3, false) OPT(3, true)
 #undef OPT
   const int smx = (int)(sizeof(double) * XWARPS * 32 * XLS);
 #define OPTX(A)                                                                                                        \
@@ -476,8 +518,10 @@ int march_init() {
   return e == cudaSuccess ? 0 : -1;
 }
 
-// One marching sweep of block B along dir (0 xi, 1 eta, 2 zeta) with accumulation mode acc.
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, bool sx) {
+// One marching sweep of block B along dir (0 xi, 1 eta, 2 zeta) with accumulation mode acc (0..2), or, with rk != null,
+// the last sweep fused with the RK stage (acc 3): the new state goes to B.r; *rk_ctas receives the number of CTAs
+// (= partial-sum groups written to rk->partials at stage 1).
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas) {
   const bool visc = c->pd.viscous != 0;
   const long long o0 = B.idx(0, 0, 0);
   MarchArgs A;
@@ -485,8 +529,10 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, bool sx) {
   A.kh = B.khat + (long long)(dir * 3) * B.M + o0;
   A.W = visc ? c->ws + (long long)(dir * 4) * B.M + o0 : nullptr;
   A.jac = B.jac + o0;
-  A.Sx = visc && sx ? c->ws + o0 : nullptr;
+  A.qn = B.qn + o0;
   A.r = B.r + o0;
+  A.partials = rk ? rk->partials : nullptr;
+  A.dt = rk ? rk->dt : 0.0; A.rk_a = rk ? rk->a : 0.0; A.rk_b = rk ? rk->b : 0.0;
   A.M = B.M;
   const int la = dir == 0 ? 1 : 0;                   // lane axis: i, except for the xi sweep (j)
   const int ta = dir == 2 ? 1 : 2;                   // third axis
@@ -494,25 +540,38 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, bool sx) {
   A.nl = B.n[la]; A.nt = B.n[ta]; A.n = B.n[dir];
   const long long lanes = (long long)A.nl * A.nt;
   const long long ctas_per_seg = (lanes + MT - 1) / MT;
-  const int nseg = pick_segments(ctas_per_seg, A.n);
+  int nseg = pick_segments(ctas_per_seg, A.n);
+  if (rk && rk->stage == 1) {
+    while (nseg > 1 && ctas_per_seg * nseg > rk->max_ctas) --nseg;
+    if (ctas_per_seg * nseg > rk->max_ctas) { c->err = "fused RK stage: block too large for the residual partials"; return CFD_E_WORKSPACE; }
+  }
   A.S = (A.n + nseg - 1) / nseg;
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;
-  if (acc == 0) launch_march_t<0>(c, A, visc);
-  else if (acc == 1) launch_march_t<1>(c, A, visc);
-  else launch_march_t<2>(c, A, visc);
+  if (rk_ctas) *rk_ctas = (int)(ctas_per_seg * ((A.n + A.S - 1) / A.S));
+#define GO(AC, ST)                                           \
+  do {                                                       \
+    if (visc) launch_march_k<AC, true, ST>(c, A);            \
+    else launch_march_k<AC, false, ST>(c, A);                \
+  } while (0)
+  if (rk) { if (rk->stage == 1) GO(3, true); else GO(3, false); }
+  else if (acc == 0) GO(0, false);
+  else if (acc == 1) GO(1, false);
+  else GO(2, false);
+#undef GO
   c->launches++;
   return 0;
 }
 
 // The xi sweep of block B as a staged marching sweep (k_march_xi) with accumulation mode acc.
 int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
-  const bool visc = false;  // the viscous xi derivative comes from k_visc_flux<true> (added by the eta sweep)
+  const bool visc = c->pd.viscous != 0;  // viscous: the flush adds S = d(Fv^xi)/d(xi) written by k_visc_flux<true>
   const long long o0 = B.idx(0, 0, 0);
   XiArgs A;
   A.q = B.q + o0;
   A.kh = B.khat + o0;
-  A.W = visc ? c->ws + o0 : nullptr;
+  A.W = nullptr;
+  A.Sx = visc ? c->ws + o0 : nullptr;
   A.jac = B.jac + o0;
   A.r = B.r + o0;
   A.M = B.M;

@@ -7,7 +7,8 @@
 #include "cfd_internal.cuh"
 #include "fastmath.cuh"
 
-int launch_sweeps(cfd_ctx* c, const BlockDev& B);
+int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas);
+__global__ void k_res_final(const double* __restrict__ partials, int n, double* __restrict__ res);
 
 // phi = (u, v, w, T = gamma p / rho) at every stored point, ghosts included (unfilled corner ghosts give
 // values nobody reads).
@@ -126,8 +127,18 @@ static void visc_geometry(const BlockDev& B, bool sxi, int* T, dim3* grid, int* 
   *grid = dim3(nrun, B.n[1] + 6, B.n[2] + 6);
 }
 
-int launch_rhs(cfd_ctx* c) {
+// cfd_rhs (fused_stage 0) or, with fused_stage 1..3 (default sweep plan only), the RHS with the RK stage fused into
+// the last sweep (cfd_stage_fused): the new state lands in the r buffers and the caller exchanges the buffer roles.
+int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
   if (c->prm.scheme != 0) { c->err = "cfd_rhs: scheme 1 (original AFWENO) is not built yet"; return CFD_E_ARG; }
+  RkFuse rk;
+  rk.stage = fused_stage;
+  rk.dt = dt;
+  rk.a = fused_stage == 2 ? 3.0 / 4.0 : (fused_stage == 3 ? 1.0 / 3.0 : 0.0);
+  rk.b = fused_stage == 2 ? 1.0 / 4.0 : (fused_stage == 3 ? 2.0 / 3.0 : 1.0);
+  double* const partials = c->ws + ws_partials_offset_doubles(c->max_M);
+  const long long cap = (long long)rk_max_partial_blocks() * (long long)c->blk.size();
+  long long used = 0;
   for (const BlockDev& B : c->blk) {
     if (c->pd.viscous) {
       double* phi = c->ws + 12 * c->max_M;
@@ -143,7 +154,17 @@ int launch_rhs(cfd_ctx* c) {
       }
       c->launches += 2;
     }
-    launch_sweeps(c, B);
+    rk.partials = partials + used * 5;
+    rk.max_ctas = cap - used < rk_max_partial_blocks() ? cap - used : rk_max_partial_blocks();
+    int ctas = 0;
+    const int rc = launch_sweeps(c, B, fused_stage ? &rk : nullptr, &ctas);
+    if (rc != 0) return rc;
+    if (fused_stage == 1) used += ctas;
+  }
+  if (fused_stage == 1) {
+    ProfScope ps(c, PK_RES);
+    k_res_final<<<1, 160, 0, c->stream>>>(partials, (int)used, c->d_res);
+    c->launches++;
   }
   CUDA_TRY(c, cudaGetLastError());
   return CFD_OK;

@@ -235,7 +235,7 @@ void launch_one(cfd_ctx* c, const BlockDev& B, bool visc) {
 }  // namespace
 
 int march_init();
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, bool sx);
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas);
 int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc);
 
 int sweep_init() {
@@ -255,7 +255,8 @@ int sweep_init() {
 // Sweep plans (cfd_set_sweep_plan): 0 = all three marching, xi through warp-private transposed staging (k_march_xi);
 // 1 = all three tiled (one thread per point);  2 = all three k_march (xi lanes run along j: uncoalesced loads);
 // 3 = xi tiled and first (plain store), eta and zeta marching (zeta applies J).
-int launch_sweeps(cfd_ctx* c, const BlockDev& B) {
+int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas) {
+  if (rk && c->sweep_plan != 0) { c->err = "fused RK stage needs sweep plan 0"; return CFD_E_ARG; }
   const bool visc = c->pd.viscous != 0;
   if (c->sweep_plan == 1) {
     { ProfScope ps(c, PK_INV_XI); launch_one<0, 0>(c, B, visc); }
@@ -263,17 +264,21 @@ int launch_sweeps(cfd_ctx* c, const BlockDev& B) {
     { ProfScope ps(c, PK_INV_ZETA); launch_one<2, 2>(c, B, visc); }
     c->launches += 3;
   } else if (c->sweep_plan == 2) {
-    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 0, false); }
-    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 1, false); }
-    { ProfScope ps(c, PK_INV_XI); launch_march(c, B, 0, 2, false); }
+    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 0, nullptr, nullptr); }
+    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 1, nullptr, nullptr); }
+    { ProfScope ps(c, PK_INV_XI); launch_march(c, B, 0, 2, nullptr, nullptr); }
   } else if (c->sweep_plan == 0) {
     { ProfScope ps(c, PK_INV_XI); launch_march_xi(c, B, 0); }
-    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, true); }
-    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 2, false); }
+    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr); }
+    {
+      ProfScope ps(c, PK_INV_ZETA);
+      const int rc = launch_march(c, B, 2, 2, rk, rk_ctas);
+      if (rc != 0) return rc;
+    }
   } else {
     { ProfScope ps(c, PK_INV_XI); launch_one<0, 0>(c, B, visc); c->launches++; }
-    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, false); }
-    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 2, false); }
+    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr); }
+    { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 2, nullptr, nullptr); }
   }
   return 0;
 }

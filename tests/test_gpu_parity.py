@@ -176,7 +176,7 @@ def test_exchange_is_bit_exact_with_signed_permutations(po, W, B):
         assert np.array_equal(g.to_numpy(b, "q", interior=False), o.field(b, "q"))
     # scramble the ghosts on the GPU, exchange again
     for b in range(8):
-        f = g.fields[b]["q"]
+        f = g.field(b, "q")
         keep = f[:, NG:-NG, NG:-NG, NG:-NG].clone()
         f.fill_(float("nan"))
         f[:, NG:-NG, NG:-NG, NG:-NG] = keep
@@ -237,6 +237,45 @@ def test_state_parity_after_steps(po, W, B, which):
         assert np.abs(g.to_numpy(0, "q") - exact).max() < 0.05
 
 
+@pytest.mark.parametrize("which", ["ragged-ns", "ragged-euler", "multiblock"])
+def test_fused_stage_matches_unfused_and_oracle(po, W, B, which):
+    """cfd_stage_fused (RK update inside the zeta sweep, buffer roles exchanged, R never stored) against cfd_stage
+    (four separate calls) and the oracle: state after 2 steps, q^n after stage 1, the stage-1 residual, and the
+    bookkeeping of cfd_buffer_roles."""
+    case = {"ragged-ns": lambda: ragged_case(W, 1), "ragged-euler": lambda: ragged_case(W, 0),
+            "multiblock": lambda: W.c4_multiblock(nb=10, mach=0.3)}[which]()
+    o, g = pair(po, B, case)
+    g2 = B.Context(case.dims, case.faces, case.params)
+    g2.load_case(case)
+    dt = o.cfl_dt(0.5)
+    assert g.buffer_roles() == (0, 1, 2)
+    ro = o.stage(1, dt, want_res=True) if hasattr(o, "stage") else None
+    rg = g.stage_fused(1, dt, want_res=True)
+    r2 = g2.stage(1, dt, want_res=True)
+    assert g.buffer_roles() == (2, 0, 1) and g2.buffer_roles() == (0, 1, 2)
+    assert np.allclose(rg, r2, rtol=1e-12)
+    if ro is not None:
+        assert np.allclose(rg, ro, rtol=1e-11)
+    for b in range(len(case.dims)):
+        assert np.array_equal(g.to_numpy(b, "qn"), g2.to_numpy(b, "qn"))  # the old q buffer, untouched
+        assert np.abs(g.to_numpy(b, "q") - g2.to_numpy(b, "q")).max() < 1e-13
+    for s in (2, 3):
+        g.stage_fused(s, dt)
+        g2.stage(s, dt)
+    assert g.buffer_roles() == (2, 0, 1)
+    g.step(dt)
+    g2.step(dt, fused=False)
+    assert sorted(g.buffer_roles()) == [0, 1, 2]
+    for b in range(len(case.dims)):
+        a, c = g.to_numpy(b, "q"), g2.to_numpy(b, "q")
+        assert np.abs(a - c).max() < 1e-12 * np.abs(c).max()
+
+    # bit-identical on repetition (fixed-order residual, no atomics)
+    g3 = B.Context(case.dims, case.faces, case.params)
+    g3.load_case(case)
+    assert np.array_equal(g3.stage_fused(1, dt, want_res=True), rg)
+
+
 def test_state_parity_after_100_steps_smooth(po, W, B):
     """north_star: 1e-10 after 100 RK3 steps on smooth cases (TGV, viscous, wavy grid; reduced to 24^3)."""
     case = W.c3_tgv(n=24, viscous=1, mach=0.1)
@@ -258,10 +297,10 @@ def subbox_check(po, g, case, b, lo, ext, S):
     sl = tuple(slice(lo[a], lo[a] + ext[a] + 2 * NG) for a in (2, 1, 0))  # array coordinates (ghost offset included)
     o = po.Oracle([tuple(ext)], [], case.params)
     for name in ("q", "khat", "jac"):
-        o.field(0, name)[...] = g.fields[b][name][(slice(None),) + sl].cpu().numpy()
+        o.field(0, name)[...] = g.field(b, name)[(slice(None),) + sl].cpu().numpy()
     o.rhs()
     isl = tuple(slice(lo[a] + NG, lo[a] + NG + ext[a]) for a in (2, 1, 0))
-    rg = g.fields[b]["r"][(slice(None),) + isl].cpu().numpy()
+    rg = g.field(b, "r")[(slice(None),) + isl].cpu().numpy()
     err = np.abs(rg - o.interior(0, "r")).max(axis=(1, 2, 3)) / S
     assert err.max() < RHS_TOL, (case.name, b, lo, err)
 
