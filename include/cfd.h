@@ -173,10 +173,13 @@ long long cfd_launch_count(const cfd_ctx*);
 int cfd_fp64_peak_probe(int iters, double* tflops);
 
 /* Kernel plan of the three inviscid sweeps inside cfd_rhs (all plans compute the same R up to summation order):
- *   0 (default) all three as marching sweeps (one thread walks a grid line segment; Q, khat staged once per point
- *     through shared memory); the xi sweep stages aligned 4-point chunks of 32 lines per warp (transposed staging);
+ *   0 (default) all three as marching sweeps (one thread walks a grid line segment; every operand staged once per
+ *     point through shared memory).  The xi sweep, whose lanes sit on lines a row pitch apart, is fed by TMA: boxes of
+ *     4 positions x 32 lines per variable land swizzled in a per-warp ring and its output leaves by TMA stores
+ *     (k_xi_tma); blocks with odd ni (row pitch not a multiple of 16 bytes) use a cp.async staging kernel instead;
  *   1 all three tiled (one thread per point);   2 all three with the plain marching kernel (the xi march reads with
- *     stride: for measurement);   3 xi tiled, eta and zeta marching. */
+ *     stride: for measurement);   3 xi tiled, eta and zeta marching;   4 plan 0 with the cp.async xi kernel forced.
+ * cfd_stage_fused needs plan 0 or 4. */
 int cfd_set_sweep_plan(cfd_ctx*, int plan);
 
 /* Device self-test of the branch-free fp64 reciprocal / reciprocal square root the hot kernels use instead

@@ -201,6 +201,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
     if ((e = cudaMemcpy(c->d_blocks_all, all.data(), sizeof(BlockDev) * all.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy blocks");
   }
   set_roles(c, 0, 1, 2);
+  xi_tma_setup(c);
   for (int p = 1; p <= 3; ++p) {
     if (c->tasks[p].empty()) continue;
     if ((e = cudaMalloc(&c->d_tasks[p], sizeof(CopyTask) * c->tasks[p].size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc tasks");
@@ -217,6 +218,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
 extern "C" int cfd_destroy(cfd_ctx* c) {
   if (!c) return CFD_OK;
   if (c->d_blocks_all) cudaFree(c->d_blocks_all);
+  xi_tma_free(c);
   for (int p = 1; p <= 3; ++p)
     if (c->d_tasks[p]) cudaFree(c->d_tasks[p]);
   if (c->d_flag) cudaFree(c->d_flag);
@@ -368,8 +370,9 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
 
 extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
   if (!c) return CFD_E_ARG;
-  if (plan < 0 || plan > 3) { c->err = "cfd_set_sweep_plan: plan must be 0..3"; return CFD_E_ARG; }
-  c->sweep_plan = plan;
+  if (plan < 0 || plan > 4) { c->err = "cfd_set_sweep_plan: plan must be 0..4"; return CFD_E_ARG; }
+  c->sweep_plan = plan == 4 ? 0 : plan;
+  c->no_tma = plan == 4;
   return CFD_OK;
 }
 

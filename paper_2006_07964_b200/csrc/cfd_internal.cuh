@@ -56,6 +56,7 @@ struct cfd_ctx {
   BlockDev* d_blocks = nullptr;       // the descriptor array of the current buffer roles (points into d_blocks_all)
   BlockDev* d_blocks_all = nullptr;   // [6][nblocks]: one array per assignment of the three state buffers to (q, qn, r)
   std::vector<double*> base[3];       // per block: the caller's q, qn, r buffers as given to cfd_create_blocks
+  void* xi_tma = nullptr;             // tensor maps of the TMA xi sweep (k_xi_tma.cu), or null
   int role[3] = {0, 1, 2};            // role[x] = which base buffer currently serves as q (x=0), qn (1), r (2)
   int* d_flag = nullptr;              // J <= 0 flag
   double* d_res = nullptr;            // 5 residual sums
@@ -65,6 +66,7 @@ struct cfd_ctx {
   long long max_M = 0;
   long long launches = 0;
   int sweep_plan = 0;                 // cfd_set_sweep_plan
+  bool no_tma = false;                // cfd_set_sweep_plan(4): plan 0 with the cp.async xi kernel even where TMA works
   std::string err;
   // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read
   bool prof_on = false;
@@ -118,6 +120,10 @@ int launch_rk(cfd_ctx* c, int stage, double dt);
 int launch_fp64_probe(int iters, double* tflops);
 int launch_fastmath_selftest(int n, const double* x_host, double* rcp_host, double* rsqrt_host);
 int sweep_init();
+void xi_tma_setup(cfd_ctx* c);
+void xi_tma_free(cfd_ctx* c);
+bool xi_tma_ok(const cfd_ctx* c, int b);
+int launch_xi_tma(cfd_ctx* c, int b);
 
 size_t ws_partials_offset_doubles(long long max_M);
 int rk_max_partial_blocks();

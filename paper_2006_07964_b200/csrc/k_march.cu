@@ -16,6 +16,7 @@
 //    (3/4, -3/20, 1/60).  Exact identity; only the summation order differs from Eq. 19 as printed.
 #include "cfd_internal.cuh"
 #include "sweep_math.cuh"
+#include "march_fir.cuh"
 #include <cmath>
 
 namespace {
@@ -49,34 +50,6 @@ __device__ __forceinline__ void cp8(double* dst, const double* src) {
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// flux-form coefficients: a_t for Eq. 19's central part, b_t for the 6th-order central difference
-#define A3 (19.0 / 3840.0)
-#define A2 (-13.0 / 320.0 + 19.0 / 3840.0)
-#define A1 (17.0 / 256.0 - 13.0 / 320.0 + 19.0 / 3840.0)
-#define B3 (1.0 / 60.0)
-#define B2 (-3.0 / 20.0 + 1.0 / 60.0)
-#define B1 (3.0 / 4.0 - 3.0 / 20.0 + 1.0 / 60.0)
-
-// one transposed-FIR update with the newest point flux x (and viscous xv); returns the filter output
-__device__ __forceinline__ double fir_push(double acc[5], double x) {
-  const double out = fma(A3, x, acc[0]);
-  acc[0] = fma(A2, x, acc[1]);
-  acc[1] = fma(A1, x, acc[2]);
-  acc[2] = fma(A1, x, acc[3]);
-  acc[3] = fma(A2, x, acc[4]);
-  acc[4] = A3 * x;
-  return out;
-}
-__device__ __forceinline__ double fir_push2(double acc[5], double x, double xv) {
-  const double out = fma(-B3, xv, fma(A3, x, acc[0]));
-  acc[0] = fma(-B2, xv, fma(A2, x, acc[1]));
-  acc[1] = fma(-B1, xv, fma(A1, x, acc[2]));
-  acc[2] = fma(-B1, xv, fma(A1, x, acc[3]));
-  acc[3] = fma(-B2, xv, fma(A2, x, acc[4]));
-  acc[4] = fma(-B3, xv, A3 * x);
-  return out;
-}
 
 // ACC 0: r = X;  1: r += X;  2: r = J (r + X);  3: the RK stage fused into the last sweep (Eq. 20):
 //   with R = J (r + X):  out = a q^n + b (q + dt R)  written to the r buffer (the caller then exchanges the roles of the
@@ -361,7 +334,7 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           double X = sX[m * XR];
-          if (VISC && m > 0) X += A.Sx[goff[t] + pos + (long long)(m - 1) * M];
+          if (VISC && m > 0) X += A.Sx[goff[t] + pos - 2 + (long long)(m - 1) * M];  // S is stored two positions to the left (k_xi_tma.cu)
           if (ACC == 0) gr[m * M] = X;
           else if (ACC == 1) gr[m * M] = gr[m * M] + X;
           else gr[m * M] = jac * (gr[m * M] + X);
@@ -469,15 +442,18 @@ void launch_march_xi_t(cfd_ctx* c, const XiArgs& A, bool visc) {
   else k_march_xi<ACC, false><<<grid, 32 * XWARPS, smem, c->stream>>>(A);
 }
 
+}  // namespace
+
 // Segment count along the sweep: enough CTAs to fill 148 SMs x 2 resident CTAs, as few partial waves as possible,
-// segments of at least 16 points (each segment repeats ~1.5 steps of prologue work).
-int pick_segments(long long ctas_per_seg, int n) {
+// segments of at least 16 points (each segment repeats ~1.5 steps of prologue work), lengths a multiple of quantum.
+int pick_segments(long long ctas_per_seg, int n, int quantum) {
   const int maxseg = n / 16 > 0 ? n / 16 : 1;
   const double slots = 148.0 * 2.0;
   int best = 1;
   double best_eff = -1.0;
   for (int ns = 1; ns <= maxseg; ++ns) {
-    const int S = (n + ns - 1) / ns;
+    int S = (n + ns - 1) / ns;
+    S = ((S + quantum - 1) / quantum) * quantum;
     const int nseg = (n + S - 1) / S;
     const double waves = (double)(ctas_per_seg * nseg) / slots;
     const double eff = waves / ceil(waves) * ((double)n / (double)(nseg * (S + 1.5)));
@@ -485,6 +461,8 @@ int pick_segments(long long ctas_per_seg, int n) {
   }
   return best;
 }
+
+namespace {
 
 template <int ACC, bool VISC, bool ST1>
 void launch_march_k(cfd_ctx* c, const MarchArgs& A) {
@@ -540,7 +518,7 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
   A.nl = B.n[la]; A.nt = B.n[ta]; A.n = B.n[dir];
   const long long lanes = (long long)A.nl * A.nt;
   const long long ctas_per_seg = (lanes + MT - 1) / MT;
-  int nseg = pick_segments(ctas_per_seg, A.n);
+  int nseg = pick_segments(ctas_per_seg, A.n, 1);
   if (rk && rk->stage == 1) {
     while (nseg > 1 && ctas_per_seg * nseg > rk->max_ctas) --nseg;
     if (ctas_per_seg * nseg > rk->max_ctas) { c->err = "fused RK stage: block too large for the residual partials"; return CFD_E_WORKSPACE; }
@@ -580,7 +558,7 @@ int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
   A.nlb = (A.nl + 31) / 32;
   A.ph = (4 - (NG & 3)) & 3;
   const long long units = (long long)A.nlb * A.nt;
-  const int nseg = pick_segments((units + XWARPS - 1) / XWARPS, A.n);
+  const int nseg = pick_segments((units + XWARPS - 1) / XWARPS, A.n, 1);
   A.S = (A.n + nseg - 1) / nseg;
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;

@@ -268,7 +268,12 @@ int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas)
     { ProfScope ps(c, PK_INV_ZETA); launch_march(c, B, 2, 1, nullptr, nullptr); }
     { ProfScope ps(c, PK_INV_XI); launch_march(c, B, 0, 2, nullptr, nullptr); }
   } else if (c->sweep_plan == 0) {
-    { ProfScope ps(c, PK_INV_XI); launch_march_xi(c, B, 0); }
+    {
+      ProfScope ps(c, PK_INV_XI);
+      const int b = (int)(&B - c->blk.data());
+      if (xi_tma_ok(c, b) && !c->no_tma) launch_xi_tma(c, b);
+      else launch_march_xi(c, B, 0);
+    }
     { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr); }
     {
       ProfScope ps(c, PK_INV_ZETA);

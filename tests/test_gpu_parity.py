@@ -79,9 +79,10 @@ def test_metrics_parity(po, W, B, which):
         assert np.abs(jg / jo - 1).max() < 1e-12
 
 
-def ragged_case(W, viscous=1):
-    """Non-cubic block whose sizes are not multiples of any tile edge (62, 6, 32): several tiles + ragged tails."""
-    n = (71, 23, 15)
+def ragged_case(W, viscous=1, n=(71, 23, 15)):
+    """Non-cubic block whose sizes are not multiples of any tile edge (62, 6, 32): several tiles + ragged tails.
+    ni odd: the xi sweep cannot use TMA (row pitch not a multiple of 16 bytes) and runs the cp.async kernel;
+    n = (70, 45, 9): TMA xi sweep with ni % 4 = 2, a partial 32-line group and several segments."""
     L = 2 * np.pi
     X, Y, Z = W._uniform_nodes(n, (L, L, L))
     modes = W.wavy_modes(11)
@@ -109,9 +110,12 @@ def test_fastmath_accuracy(B):
 # ------------------------------------------------------------------------------------------------
 # S2 + S3: RHS parity, element by element
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("which", ["c1-euler", "tgv-ns", "ragged-ns", "ragged-euler", "multiblock-ns", "cylinder-ns", "tiny"])
+@pytest.mark.parametrize("which", ["c1-euler", "tgv-ns", "ragged-ns", "ragged-euler", "ragged-even-ns", "ragged-even-euler",
+                                   "multiblock-ns", "cylinder-ns", "tiny"])
 def test_rhs_parity(po, W, B, which):
     case = {"c1-euler": lambda: W.c1_vortex(32),
+            "ragged-even-ns": lambda: ragged_case(W, 1, n=(70, 45, 9)),
+            "ragged-even-euler": lambda: ragged_case(W, 0, n=(70, 45, 9)),
             "tgv-ns": lambda: W.tgv_sine_box(24, viscous=1, mach=0.4),
             "ragged-ns": lambda: ragged_case(W, 1),
             "ragged-euler": lambda: ragged_case(W, 0),
@@ -122,11 +126,11 @@ def test_rhs_parity(po, W, B, which):
     assert_rhs_parity(o, g, case)
 
 
-@pytest.mark.parametrize("plan", [1, 2])
+@pytest.mark.parametrize("plan", [1, 2, 3, 4])
 @pytest.mark.parametrize("which", ["ragged-ns", "ragged-euler", "multiblock-ns", "cylinder-ns", "tiny"])
 def test_rhs_parity_other_sweep_plans(po, W, B, which, plan):
-    """cfd_set_sweep_plan: all-tiled (1) and all-marching (2) sweeps against the oracle (plan 0 is the default
-    everywhere else)."""
+    """cfd_set_sweep_plan: all-tiled (1), all k_march (2), xi tiled + marching (3) and the default plan with the
+    cp.async xi kernel forced (4) against the oracle (plan 0 is the default everywhere else)."""
     case = {"ragged-ns": lambda: ragged_case(W, 1),
             "ragged-euler": lambda: ragged_case(W, 0),
             "multiblock-ns": lambda: W.c4_multiblock(nb=12, mach=0.3),
