@@ -370,9 +370,9 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
 
 extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
   if (!c) return CFD_E_ARG;
-  if (plan < 0 || plan > 4) { c->err = "cfd_set_sweep_plan: plan must be 0..4"; return CFD_E_ARG; }
-  c->sweep_plan = plan == 4 ? 0 : plan;
-  c->no_tma = plan == 4;
+  if (plan < 0 || plan > 5) { c->err = "cfd_set_sweep_plan: plan must be 0..5"; return CFD_E_ARG; }
+  c->sweep_plan = plan >= 4 ? 0 : plan;
+  c->xi_mode = plan == 4 ? 2 : (plan == 5 ? 1 : 0);
   return CFD_OK;
 }
 

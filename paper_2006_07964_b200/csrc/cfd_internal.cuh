@@ -66,7 +66,7 @@ struct cfd_ctx {
   long long max_M = 0;
   long long launches = 0;
   int sweep_plan = 0;                 // cfd_set_sweep_plan
-  bool no_tma = false;                // cfd_set_sweep_plan(4): plan 0 with the cp.async xi kernel even where TMA works
+  int xi_mode = 0;                    // plan 0 xi kernel: 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
   std::string err;
   // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read
   bool prof_on = false;
@@ -123,7 +123,8 @@ int sweep_init();
 void xi_tma_setup(cfd_ctx* c);
 void xi_tma_free(cfd_ctx* c);
 bool xi_tma_ok(const cfd_ctx* c, int b);
-int launch_xi_tma(cfd_ctx* c, int b);
+bool xi_ldg_ok(const cfd_ctx* c, int b);
+int launch_xi_tma(cfd_ctx* c, int b, bool tma);
 
 size_t ws_partials_offset_doubles(long long max_M);
 int rk_max_partial_blocks();

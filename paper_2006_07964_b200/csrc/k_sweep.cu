@@ -271,7 +271,8 @@ int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas)
     {
       ProfScope ps(c, PK_INV_XI);
       const int b = (int)(&B - c->blk.data());
-      if (xi_tma_ok(c, b) && !c->no_tma) launch_xi_tma(c, b);
+      if (c->xi_mode == 1 && xi_tma_ok(c, b)) launch_xi_tma(c, b, true);
+      else if (c->xi_mode != 2 && xi_ldg_ok(c, b)) launch_xi_tma(c, b, false);
       else launch_march_xi(c, B, 0);
     }
     { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr); }

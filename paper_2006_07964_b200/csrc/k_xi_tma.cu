@@ -284,6 +284,163 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
   flush((last3 + NG) >> 2);
   if (lane == 0) tma_wait0();
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// The same sweep with the ring filled by warp-cooperative 16-byte cp.async instead of TMA.  Measured on B200 the TMA
+// unit spends ~5 cycles per 32-byte box row (6 B/cycle/SM), which makes the TMA variant TMA-bound (1.41 ms at 256^3);
+// 16-byte LDGSTS with lane -> (line l/2 + 16t, half l%2) writes the same swizzled layout (the XOR done by hand), two
+// lanes cover one sector of a line and a quarter warp writes 128 contiguous bytes.  The flush uses the same lane
+// mapping: LDS.128 of the parked outputs (+ S from its buffer), STG.128 to r.
+struct XiLArgs {
+  const double* q;    // array origin (ghosts included) of the current q
+  const double* kh;   // khat^xi rows
+  const double* sx;   // S rows (workspace), stored two positions to the left
+  double* r;
+  long long M, s1, s2;  // variable, j, k strides (doubles)
+  XiTArgs g;
+};
+
+__device__ __forceinline__ void cp16(char* dst, const double* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+
+template <bool VISC>
+__global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
+  extern __shared__ char smem_raw[];
+  const XiTArgs& A = L.g;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const long long unit = (long long)blockIdx.x * TW + wid;
+  const int lb = (int)(unit % A.nlb);
+  const int it = (int)(unit / A.nlb);
+  if (it >= A.nt) return;  // warp-uniform; the kernel has no CTA-wide barrier
+  const int p0 = blockIdx.y * A.S;  // multiple of 4
+  const int p1 = min(A.n, p0 + A.S);
+  char* const base = smem_raw + ((256u - (smem_u32(smem_raw) & 255u)) & 255u);
+  char* const ring = base + wid * WARP_BYTES;
+  char* const sxbuf = ring + 3 * SLOT;
+  const int swz = (lane >> 2) & 1;
+  const int off0 = lane * 32 + (swz << 4), off1 = lane * 32 + ((swz ^ 1) << 4);
+  auto pair_ptr = [&](int pn) -> char* { return ring + ((pn >> 1) % 3) * SLOT + ((pn & 1) ? off1 : off0); };
+  // loader / flusher role: lines lsub + 16 t (t = 0, 1), half lh of the chunk
+  const int lsub = lane >> 1, lh = lane & 1;
+  long long goff[2];
+  bool lok[2];
+  int soff[2];
+#pragma unroll
+  for (int t = 0; t < 2; ++t) {
+    const int ln = lsub + 16 * t;                     // line within the warp's group
+    const int jl = lb * 32 + ln;                      // interior j of that line
+    lok[t] = jl < A.nl;
+    goff[t] = (long long)(it + NG) * L.s2 + (long long)(min(jl, A.nl - 1) + NG) * L.s1 + 2 * lh;
+    soff[t] = ln * 32 + ((lh ^ ((ln >> 2) & 1)) << 4);
+  }
+  const long long M = L.M;
+  auto load_chunk = [&](int ch) {
+    char* const slot = ring + (ch % 3) * SLOT;
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+      const long long g = goff[t] + ch * 4;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) cp16(slot + m * PLANE + soff[t], L.q + m * M + g);
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc) cp16(slot + (5 + cc) * PLANE + soff[t], L.kh + cc * M + g);
+    }
+  };
+  auto load_sx = [&](int ch) {
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+      const long long g = goff[t] + ch * 4;
+#pragma unroll
+      for (int m = 0; m < 4; ++m) cp16(sxbuf + m * PLANE + soff[t], L.sx + m * M + g);
+    }
+  };
+  // r array positions 4 ch + 2 .. 4 ch + 5 are parked in the Q planes of chunk ch
+  auto flush = [&](int ch, int rlo, int rhi) {  // only r positions in [rlo, rhi) are written
+    const char* const slot = ring + (ch % 3) * SLOT;
+    const int rp = ch * 4 + 2 + 2 * lh - NG;  // first of my two r positions
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+      if (!lok[t]) continue;
+      double* const gr = L.r + goff[t] + ch * 4 + 2;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) {
+        double2 v = *reinterpret_cast<const double2*>(slot + m * PLANE + soff[t]);
+        if (VISC && m > 0) {
+          const double2 sv = *reinterpret_cast<const double2*>(sxbuf + (m - 1) * PLANE + soff[t]);
+          v.x += sv.x; v.y += sv.y;
+        }
+        if (rp >= rlo && rp + 1 < rhi) *reinterpret_cast<double2*>(gr + m * M) = v;
+        else {
+          if (rp >= rlo && rp < rhi) gr[m * M] = v.x;
+          if (rp + 1 >= rlo && rp + 1 < rhi) gr[m * M + 1] = v.y;
+        }
+      }
+    }
+  };
+
+  const int a0 = p0 - 1 + NG;
+  const int ch0 = a0 >> 2;
+  load_chunk(ch0 - 1); load_chunk(ch0);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  load_chunk(ch0 + 1);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  XiState st;
+#pragma unroll
+  for (int m = 0; m < 5; ++m) {
+#pragma unroll
+    for (int t = 0; t < 5; ++t) st.acc[m][t] = 0.0;
+    st.ULc[m] = 0.0; st.Phip[m] = 0.0;
+  }
+  asm volatile("cp.async.wait_group 1;" ::: "memory");
+  __syncwarp();
+  const int pb0 = (a0 - 3) >> 1;
+  char* P0 = pair_ptr(pb0);
+  char* P1 = pair_ptr(pb0 + 1);
+  char* P2 = pair_ptr(pb0 + 2);
+  char* P3 = P2;
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const char* P = t == 0 ? P0 : (t == 3 ? P2 : P1);
+    double v[8];
+#pragma unroll
+    for (int x = 0; x < 8; ++x) v[x] = (t == 0 || t == 2) ? LD2(P, x).y : LD2(P, x).x;
+    double F[5];
+    point_flux(v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7], A.gamma, F);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) fir_push(st.acc[m], F[m]);
+  }
+  const double gamma = A.gamma, eps4 = A.eps4;
+  int last3 = -1;
+  for (int j = p0 - 1; j <= p1; j += 2) {
+    const int a = j + NG;  // odd
+    if ((a & 3) == 3) {
+      // flush the chunk before chunk(a) (its parks are complete), then refill its slot with the chunk two ahead and
+      // fetch S for the chunk being parked now
+      __syncwarp();
+      if (j >= p0 + 5) flush((a >> 2) - 1, p0, p1);
+      const int cn = (a >> 2) + 2;
+      if (cn * 4 <= p1 + NG + 2) load_chunk(cn);
+      if (VISC) load_sx(a >> 2);
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      last3 = j;
+    }
+    xi_step<1>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4);
+    if (j + 1 <= p1) {
+      const int a1 = a + 1;
+      if ((a1 & 3) == 2) {  // position a1+2 opens the next chunk
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+      }
+      P3 = pair_ptr(pb0 + ((j - (p0 - 1)) >> 1) + 3);
+      xi_step<0>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4);
+      P0 = P1; P1 = P2; P2 = P3;
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncwarp();
+  flush((last3 + NG) >> 2, p0, p1);
+}
+
 #undef LD2
 
 // ---- host side: tensor maps (one per state buffer and block, plus khat^xi and S) and the launcher ----
@@ -295,6 +452,7 @@ struct XiMaps {
 };
 struct XiTmaState {
   std::vector<XiMaps> maps;
+  bool ldg_ok = false;
 };
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -307,7 +465,7 @@ bool encode(EncodeTiledFn fn, CUtensorMap* tm, const BlockDev& B, double* basep,
   const cuuint32_t box[4] = {4, 32, 1, (cuuint32_t)nvar};
   const cuuint32_t es[4] = {1, 1, 1, 1};
   return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, basep, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace
@@ -318,6 +476,12 @@ void xi_tma_setup(cfd_ctx* c) {
   XiTmaState* S = new XiTmaState;
   S->maps.resize(c->blk.size());
   c->xi_tma = S;
+  if (cudaFuncSetAttribute(k_xi_ldg<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_xi_ldg<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess) {
+    cudaGetLastError();
+    return;
+  }
+  S->ldg_ok = true;
   EncodeTiledFn fn = nullptr;
   cudaDriverEntryPointQueryResult qr;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&fn, cudaEnableDefault, &qr) != cudaSuccess || !fn ||
@@ -351,11 +515,17 @@ bool xi_tma_ok(const cfd_ctx* c, int b) {
   const XiTmaState* S = static_cast<const XiTmaState*>(c->xi_tma);
   return S && S->maps[b].ok;
 }
+// the 16-byte cp.async variant needs an even row pitch (16-byte aligned position pairs) and ni >= 8
+bool xi_ldg_ok(const cfd_ctx* c, int b) {
+  const XiTmaState* S = static_cast<const XiTmaState*>(c->xi_tma);
+  return S && S->ldg_ok && !(c->blk[b].m[0] & 1) && c->blk[b].n[0] >= 8;
+}
 
 int pick_segments(long long ctas_per_seg, int n, int quantum);
 
-// The xi sweep of block b (r = X + S) with the TMA marching kernel.
-int launch_xi_tma(cfd_ctx* c, int b) {
+// The xi sweep of block b (r = X + S) with the chunk-ring marching kernel; tma: fill the ring by TMA (k_xi_tma),
+// else by 16-byte cp.async (k_xi_ldg, the default: the TMA unit is the bottleneck for 32-byte box rows).
+int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
   const XiTmaState* S = static_cast<const XiTmaState*>(c->xi_tma);
   const XiMaps& X = S->maps[b];
   const BlockDev& B = c->blk[b];
@@ -369,6 +539,16 @@ int launch_xi_tma(cfd_ctx* c, int b) {
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;
   dim3 grid((unsigned)ctas, (unsigned)((A.n + A.S - 1) / A.S));
+  if (!tma) {
+    XiLArgs L;
+    L.q = B.q; L.kh = B.khat; L.sx = c->ws; L.r = B.r;
+    L.M = B.M; L.s1 = B.s[1]; L.s2 = B.s[2];
+    L.g = A;
+    if (c->pd.viscous) k_xi_ldg<true><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);
+    else k_xi_ldg<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);
+    c->launches++;
+    return 0;
+  }
   const CUtensorMap& tq = X.st[c->role[0]];
   const CUtensorMap& tr = X.st[c->role[2]];
   if (c->pd.viscous) k_xi_tma<true><<<grid, 32 * TW, XT_SMEM, c->stream>>>(tq, X.kh, tr, X.sx, A);
