@@ -34,6 +34,7 @@ struct MarchArgs {
   const double* W;      // viscous flux rows of direction d, + interior origin (VISC)
   const double* jac;    // + interior origin (ACC 2)
   const double* qn;     // q^n + interior origin (ACC 3, stages 2 and 3)
+  const double* Sx;     // SX: S = d(Fv^xi)/d(xi) rows 2..5 (k_visc_flux<true>), + interior origin
   double* r;            // + interior origin
   double* partials;     // ACC 3 stage 1: 5 partial sums of R_m^2 per CTA
   long long M;          // plane stride between variables
@@ -60,22 +61,25 @@ __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0
 // Every operand arrives through thread-private shared-memory columns filled by cp.async one step ahead (Q, khat of
 // position j+3; the viscous rows of j+3; old r, J, q^n of the output position): nothing is held in registers across
 // a step, which is what the register allocation of this kernel (~250 registers, 2 CTAs per SM) needs.
-template <int ACC, bool ST1>
+template <int ACC, bool ST1, bool SX>
 struct OutCfg {
   static constexpr int O_R = 0;                                  // old r (5), ACC >= 1
   static constexpr int O_J = ACC >= 1 ? 5 : 0;                   // J (1), ACC >= 2
   static constexpr int O_QN = O_J + (ACC >= 2 ? 1 : 0);          // q^n (5), ACC 3 stages 2, 3
-  static constexpr int NOUT = O_QN + ((ACC == 3 && !ST1) ? 5 : 0);
+  static constexpr int O_S = O_QN + ((ACC == 3 && !ST1) ? 5 : 0);  // S = d(Fv^xi)/d(xi) rows 2..5 (4), SX
+  static constexpr int NOUT = O_S + (SX ? 4 : 0);
 };
-template <int ACC, bool VISC, bool ST1>
+template <int ACC, bool VISC, bool ST1, bool SX>
 constexpr int march_smem_doubles() {
-  return (RING * RV + (VISC ? 8 : 0) + 2 * OutCfg<ACC, ST1>::NOUT + ((ACC == 3 && ST1) ? 5 : 0)) * MT;
+  return (RING * RV + (VISC ? 8 : 0) + 2 * OutCfg<ACC, ST1, SX>::NOUT + ((ACC == 3 && ST1) ? 5 : 0)) * MT;
 }
 
-template <int ACC, bool VISC, bool ST1>
+// SX (with ACC >= 1): the viscous xi term S written by k_visc_flux<true> is added to r here (the xi sweep runs first
+// and knows nothing about viscosity).
+template <int ACC, bool VISC, bool ST1, bool SX>
 __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
   extern __shared__ double ring[];  // thread-private columns: [RING][RV][MT] | W [2][4][MT] | out operands [2][NOUT][MT] | res [5][MT]
-  using OC = OutCfg<ACC, ST1>;
+  using OC = OutCfg<ACC, ST1, SX>;
   constexpr int NOUT = OC::NOUT;
   const int tid = threadIdx.x;
   const long long L = (long long)blockIdx.x * MT + tid;
@@ -125,6 +129,10 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
       if (ACC == 3 && !ST1) {
 #pragma unroll
         for (int m = 0; m < 5; ++m) cp8(s + (OC::O_QN + m) * MT, A.qn + base + m * M + o);
+      }
+      if (SX) {
+#pragma unroll
+        for (int m = 0; m < 4; ++m) cp8(s + (OC::O_S + m) * MT, A.Sx + base + m * M + o);
       }
     };
     // ---- prologue: positions p0-4 .. p0+1 (first step j = p0-1 reads Q j-2..j+2 and khat j-3..j+2) ----
@@ -201,7 +209,7 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
             const double X = Phip[m] - Phi;
             double* rp = r + m * M + (long long)(j - 1) * sm;
             if (ACC == 0) *rp = X;
-            else if (ACC == 1) *rp = so[(OC::O_R + m) * MT] + X;
+            else if (ACC == 1) *rp = (SX && m > 0) ? (so[(OC::O_R + m) * MT] + so[(OC::O_S + m - 1) * MT]) + X : so[(OC::O_R + m) * MT] + X;
             else if (ACC == 2) *rp = jac * (so[(OC::O_R + m) * MT] + X);
             else {
               const double R = jac * (so[(OC::O_R + m) * MT] + X);
@@ -334,7 +342,6 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           double X = sX[m * XR];
-          if (VISC && m > 0) X += A.Sx[goff[t] + pos - 2 + (long long)(m - 1) * M];  // S is stored two positions to the left (k_xi_tma.cu)
           if (ACC == 0) gr[m * M] = X;
           else if (ACC == 1) gr[m * M] = gr[m * M] + X;
           else gr[m * M] = jac * (gr[m * M] + X);
@@ -464,18 +471,18 @@ int pick_segments(long long ctas_per_seg, int n, int quantum) {
 
 namespace {
 
-template <int ACC, bool VISC, bool ST1>
+template <int ACC, bool VISC, bool ST1, bool SX = false>
 void launch_march_k(cfd_ctx* c, const MarchArgs& A) {
   const long long lanes = (long long)A.nl * A.nt;
   dim3 grid((unsigned)((lanes + MT - 1) / MT), (unsigned)((A.n + A.S - 1) / A.S));
-  const size_t smem = sizeof(double) * march_smem_doubles<ACC, VISC, ST1>();
-  k_march<ACC, VISC, ST1><<<grid, MT, smem, c->stream>>>(A);
+  const size_t smem = sizeof(double) * march_smem_doubles<ACC, VISC, ST1, SX>();
+  k_march<ACC, VISC, ST1, SX><<<grid, MT, smem, c->stream>>>(A);
 }
 
-template <int ACC, bool VISC, bool ST1>
+template <int ACC, bool VISC, bool ST1, bool SX = false>
 cudaError_t march_attr() {
-  return cudaFuncSetAttribute(k_march<ACC, VISC, ST1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)(sizeof(double) * march_smem_doubles<ACC, VISC, ST1>()));
+  return cudaFuncSetAttribute(k_march<ACC, VISC, ST1, SX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)(sizeof(double) * march_smem_doubles<ACC, VISC, ST1, SX>()));
 }
 
 }  // namespace
@@ -487,6 +494,7 @@ int march_init() {
   if (e == cudaSuccess) e = march_attr<A, false, S>();
   OPT(0, false) OPT(1, false) OPT(2, false) OPT(3, false) OPT(3, true)
 #undef OPT
+  if (e == cudaSuccess) e = march_attr<1, true, false, true>();
   const int smx = (int)(sizeof(double) * XWARPS * 32 * XLS);
 #define OPTX(A)                                                                                                        \
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi<A, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx); \
@@ -499,7 +507,7 @@ int march_init() {
 // One marching sweep of block B along dir (0 xi, 1 eta, 2 zeta) with accumulation mode acc (0..2), or, with rk != null,
 // the last sweep fused with the RK stage (acc 3): the new state goes to B.r; *rk_ctas receives the number of CTAs
 // (= partial-sum groups written to rk->partials at stage 1).
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas) {
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas, bool sx) {
   const bool visc = c->pd.viscous != 0;
   const long long o0 = B.idx(0, 0, 0);
   MarchArgs A;
@@ -508,6 +516,7 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
   A.W = visc ? c->ws + (long long)(dir * 4) * B.M + o0 : nullptr;
   A.jac = B.jac + o0;
   A.qn = B.qn + o0;
+  A.Sx = c->ws + o0;
   A.r = B.r + o0;
   A.partials = rk ? rk->partials : nullptr;
   A.dt = rk ? rk->dt : 0.0; A.rk_a = rk ? rk->a : 0.0; A.rk_b = rk ? rk->b : 0.0;
@@ -534,6 +543,7 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
   } while (0)
   if (rk) { if (rk->stage == 1) GO(3, true); else GO(3, false); }
   else if (acc == 0) GO(0, false);
+  else if (acc == 1 && sx && visc) launch_march_k<1, true, false, true>(c, A);
   else if (acc == 1) GO(1, false);
   else GO(2, false);
 #undef GO
@@ -543,7 +553,7 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
 
 // The xi sweep of block B as a staged marching sweep (k_march_xi) with accumulation mode acc.
 int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
-  const bool visc = c->pd.viscous != 0;  // viscous: the flush adds S = d(Fv^xi)/d(xi) written by k_visc_flux<true>
+  const bool visc = false;  // the viscous xi term S is added by the eta sweep
   const long long o0 = B.idx(0, 0, 0);
   XiArgs A;
   A.q = B.q + o0;

@@ -33,9 +33,8 @@ __device__ __forceinline__ double d6c(double m3, double m2, double m1, double p1
 // direction (the only one ever differentiated there).
 // One CTA = one run of T points along i (plus 3 on either side) at fixed (j, k).  SXI: the xi flux rows stay in
 // shared memory and the CTA writes their 6th-order central xi-derivative S = d(Fv^xi)/d(xi) on interior
-// points instead of the rows themselves (rows W[0..3], stored TWO POSITIONS TO THE LEFT, at i-2, so that the aligned
-// 4-point chunks of S coincide with the chunks in which the xi sweep parks its outputs, k_xi_tma.cu); the xi sweep
-// adds S to r when it writes r.  !SXI: the xi rows are written as they are (sweep plans 1-3 differentiate them in the xi sweep).
+// points instead of the rows themselves (rows W[0..3]); the eta sweep adds S to r (the xi marching sweep then needs
+// no viscous input).  !SXI: the xi rows are written as they are (sweep plans 1-3 differentiate them in the xi sweep).
 template <bool SXI>
 __global__ void __launch_bounds__(256) k_visc_flux(BlockDev B, ParamsDev P, const double* __restrict__ phi, double* __restrict__ W,
                                                    int T) {
@@ -114,7 +113,7 @@ __global__ void __launch_bounds__(256) k_visc_flux(BlockDev B, ParamsDev P, cons
       const long long p = B.idx(i, j, k);
 #pragma unroll
       for (int m = 0; m < 4; ++m)
-        W[(long long)m * M + p - 2] = d6c(sW[m][t - 3], sW[m][t - 2], sW[m][t - 1], sW[m][t + 1], sW[m][t + 2], sW[m][t + 3]);
+        W[(long long)m * M + p] = d6c(sW[m][t - 3], sW[m][t - 2], sW[m][t - 1], sW[m][t + 1], sW[m][t + 2], sW[m][t + 3]);
     }
   }
 }

@@ -235,7 +235,7 @@ void launch_one(cfd_ctx* c, const BlockDev& B, bool visc) {
 }  // namespace
 
 int march_init();
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas);
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas, bool sx = false);
 int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc);
 
 int sweep_init() {
@@ -275,7 +275,7 @@ int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas)
       else if (c->xi_mode != 2 && xi_ldg_ok(c, b)) launch_xi_tma(c, b, false);
       else launch_march_xi(c, B, 0);
     }
-    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr); }
+    { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr, true); }
     {
       ProfScope ps(c, PK_INV_ZETA);
       const int rc = launch_march(c, B, 2, 2, rk, rk_ctas);

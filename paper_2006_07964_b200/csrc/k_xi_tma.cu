@@ -544,15 +544,13 @@ int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
     L.q = B.q; L.kh = B.khat; L.sx = c->ws; L.r = B.r;
     L.M = B.M; L.s1 = B.s[1]; L.s2 = B.s[2];
     L.g = A;
-    if (c->pd.viscous) k_xi_ldg<true><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);
-    else k_xi_ldg<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);
+    k_xi_ldg<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);  // S is added by the eta sweep
     c->launches++;
     return 0;
   }
   const CUtensorMap& tq = X.st[c->role[0]];
   const CUtensorMap& tr = X.st[c->role[2]];
-  if (c->pd.viscous) k_xi_tma<true><<<grid, 32 * TW, XT_SMEM, c->stream>>>(tq, X.kh, tr, X.sx, A);
-  else k_xi_tma<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(tq, X.kh, tr, X.sx, A);
+  k_xi_tma<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(tq, X.kh, tr, X.sx, A);  // S is added by the eta sweep
   c->launches++;
   return 0;
 }
