@@ -301,7 +301,7 @@ struct XiLArgs {
 };
 
 __device__ __forceinline__ void cp16(char* dst, const double* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+  asm volatile("cp.async.cg.shared.global.L2::128B [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
 
 template <bool VISC>
