@@ -210,7 +210,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   }
   if ((e = cudaMalloc(&c->d_flag, sizeof(int))) != cudaSuccess) return cuda_fail(e, "cudaMalloc flag");
   if ((e = cudaMalloc(&c->d_res, sizeof(double) * 8)) != cudaSuccess) return cuda_fail(e, "cudaMalloc res");
-  if (sweep_init() != 0) return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute (dynamic shared memory of the sweep kernels)");
+  if (sweep_init() != 0 || visc_march_init() != 0) return cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute (dynamic shared memory of the sweep kernels)");
   *out = c;
   return CFD_OK;
 }
@@ -370,8 +370,9 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
 
 extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
   if (!c) return CFD_E_ARG;
-  if (plan < 0 || plan > 5) { c->err = "cfd_set_sweep_plan: plan must be 0..5"; return CFD_E_ARG; }
+  if (plan < 0 || plan > 6) { c->err = "cfd_set_sweep_plan: plan must be 0..6"; return CFD_E_ARG; }
   c->sweep_plan = plan >= 4 ? 0 : plan;
+  c->visc_tiled = plan == 6;
   c->xi_mode = plan == 4 ? 2 : (plan == 5 ? 1 : 0);
   return CFD_OK;
 }

@@ -66,6 +66,7 @@ struct cfd_ctx {
   long long max_M = 0;
   long long launches = 0;
   int sweep_plan = 0;                 // cfd_set_sweep_plan
+  bool visc_tiled = false;            // cfd_set_sweep_plan(6): plan 0 with k_phi + k_visc_flux instead of k_visc_march
   int xi_mode = 0;                    // plan 0 xi kernel: 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
   std::string err;
   // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read
@@ -120,6 +121,8 @@ int launch_rk(cfd_ctx* c, int stage, double dt);
 int launch_fp64_probe(int iters, double* tflops);
 int launch_fastmath_selftest(int n, const double* x_host, double* rcp_host, double* rsqrt_host);
 int sweep_init();
+int visc_march_init();
+int launch_visc_march(cfd_ctx* c, const BlockDev& B);
 void xi_tma_setup(cfd_ctx* c);
 void xi_tma_free(cfd_ctx* c);
 bool xi_tma_ok(const cfd_ctx* c, int b);

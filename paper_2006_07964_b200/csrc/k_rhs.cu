@@ -140,7 +140,10 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
   const long long cap = (long long)rk_max_partial_blocks() * (long long)c->blk.size();
   long long used = 0;
   for (const BlockDev& B : c->blk) {
-    if (c->pd.viscous) {
+    if (c->pd.viscous && c->sweep_plan == 0 && !c->visc_tiled) {
+      ProfScope ps(c, PK_VISC_FLUX);
+      launch_visc_march(c, B);
+    } else if (c->pd.viscous) {
       double* phi = c->ws + 12 * c->max_M;
       { ProfScope ps(c, PK_VISC_PHI); k_phi<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, c->pd.gamma, phi); }
       const bool sxi = c->sweep_plan == 0;

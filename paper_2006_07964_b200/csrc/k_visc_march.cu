@@ -1,0 +1,217 @@
+// S3 up to the point fluxes as ONE k-marching kernel (replaces k_phi + k_visc_flux<true> on the default plan).
+// sm_100a, fp64.  P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.  Shares no code with oracle/.
+//
+// k_visc_flux reads 72 neighbour values of phi per point through L1 (latency-bound: DRAM 44 %, LSU wavefronts 62 %) and
+// needs phi stored by a separate pass.  Here a CTA owns a tile of (i, j) columns and marches along k:
+//   * phi = (u, v, w, T) is computed from Q on the fly and never stored;
+//   * the zeta stencil lives in REGISTERS: each thread keeps phi of its own column at k-3 .. k+3 (28 doubles);
+//   * the (i, j) plane of phi at k (tile + halo of 3 in j, 6 in i) lives in SHARED memory, double buffered: the xi and
+//     eta stencils read it with LDS;
+//   * Q of plane k+4, the halo cells of plane k+1 and the ten metric values of plane k+1 arrive by cp.async in
+//     thread-private shared-memory slots one step ahead (no registers held across a step);
+//   * the xi rows of the flux go to shared memory and come back as S = d(Fv^xi)/d(xi), as in k_visc_flux<true>.
+// Output (workspace rows): W[0..3] = S on interior points; W[4..7] = Fv^eta rows 2..5 on (i, k) interior, j in [-3, nj+3);
+// W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).  Same arithmetic per point as k_phi + k_visc_flux.
+#include "cfd_internal.cuh"
+#include "fastmath.cuh"
+
+namespace {
+
+constexpr int VX = 64, VY = 8;          // threads: columns i0-3 .. i0+60, rows j0 .. j0+7
+constexpr int PC = VX + 6 + 2;          // plane columns i0-6 .. i0+63 (70), padded to 72
+constexpr int PR = VY + 6;              // plane rows j0-3 .. j0+10
+constexpr int NHALO = 2 * 3 * VX + 2 * 3 * VY;  // halo cells of the plane: 432
+constexpr int NT = VX * VY;
+// shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [4][VY][VX] | Q stage [5][NT] | halo stage [5][NT] | metric stage [10][NT]
+constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 4 * NT, SM_Q = 5 * NT, SM_H = 5 * NT, SM_M = 10 * NT;
+constexpr int VM_SMEM = (SM_PHI + SM_WX + SM_Q + SM_H + SM_M) * 8;
+
+__device__ __forceinline__ void vcp8(double* dst, const double* src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
+}
+__device__ __forceinline__ double vd6c(double m3, double m2, double m1, double p1, double p2, double p3) {
+  return (3.0 / 4.0) * (p1 - m1) - (3.0 / 20.0) * (p2 - m2) + (1.0 / 60.0) * (p3 - m3);
+}
+// phi = (u, v, w, T = gamma p / rho) from the conservative state: the arithmetic of k_phi
+__device__ __forceinline__ void phi_of(double r, double m1, double m2, double m3, double e, double gamma, double f[4]) {
+  const double ir = frcp(r);
+  const double u = m1 * ir, v = m2 * ir, w = m3 * ir;
+  const double pr = (gamma - 1.0) * fma(-0.5 * r, fma(u, u, fma(v, v, w * w)), e);
+  f[0] = u; f[1] = v; f[2] = w; f[3] = (gamma * pr) * ir;
+}
+
+__global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, double* __restrict__ W, int TI, int KS) {
+  extern __shared__ double vsm[];
+  double* const sphi = vsm;               // [2][4][PR][PC]
+  double* const swx = sphi + SM_PHI;      // [4][VY][VX]
+  double* const sq = swx + SM_WX;         // [5][NT]
+  double* const sh = sq + SM_Q;           // [5][NT]
+  double* const smt = sh + SM_H;          // [10][NT]
+  const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * VX + tx;
+  const int i0 = blockIdx.x * TI, j0 = -3 + (int)blockIdx.y * VY;
+  const int kb = -3 + (int)blockIdx.z * KS, ke = min(kb + KS, B.n[2] + 3);
+  const int i = i0 - 3 + tx, j = j0 + ty;
+  const long long M = B.M, s1 = B.s[1], s2 = B.s[2];
+  const double gamma = P.gamma;
+  // my column: inside the array?  (plane filler)   which results are wanted from it?
+  const bool col_in = (i + NG < B.m[0]) && (j + NG < B.m[1]);
+  const bool oi = i < 0 || i >= B.n[0], oj = j < 0 || j >= B.n[1];
+  const bool own = tx >= 3 && tx < TI + 3 && i < B.n[0];                       // point-wise outputs are mine
+  const bool want_xi = tx < TI + 6 && i < B.n[0] + 3 && !oj;                    // xi rows (k interior)
+  const bool want_eta = own && j < B.n[1] + 3;                                  // eta rows (k interior)
+  const bool want_zeta = own && !oj;                                            // zeta rows (all k of the march)
+  const bool any = col_in && (want_xi || want_eta || want_zeta) && !(oi && oj);
+  const long long pcol = (long long)(j + NG) * s1 + (i + NG);                  // array offset of (i, j, k = -NG)
+  // my halo cell of the plane (if any): top band, bottom band, left columns, right columns
+  int hc = -1, hr = -1;  // plane column / row
+  if (tid < 3 * VX) { hr = tid / VX; hc = 3 + tid % VX; }
+  else if (tid < 6 * VX) { hr = VY + 3 + (tid - 3 * VX) / VX; hc = 3 + tid % VX; }
+  else if (tid < 6 * VX + 3 * VY) { hr = 3 + (tid - 6 * VX) / 3; hc = (tid - 6 * VX) % 3; }
+  else if (tid < NHALO) { hr = 3 + (tid - 6 * VX - 3 * VY) / 3; hc = VX + 3 + (tid - 6 * VX - 3 * VY) % 3; }
+  const int hi = i0 - 6 + hc, hj = j0 - 3 + hr;
+  const bool halo_in = hc >= 0 && hi + NG >= 0 && hi + NG < B.m[0] && hj + NG >= 0 && hj + NG < B.m[1];
+  const long long phal = (long long)(hj + NG) * s1 + (hi + NG);
+
+  auto stage = [&](int k) {  // cp.async for the step of plane k: Q(k+3) of my column, my halo cell at k, metrics at k
+    if (col_in && k + 3 + NG < B.m[2]) {
+      const long long o = pcol + (long long)(k + 3 + NG) * s2;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) vcp8(sq + m * NT + tid, B.q + m * M + o);
+    }
+    if (halo_in) {
+      const long long o = phal + (long long)(k + NG) * s2;
+#pragma unroll
+      for (int m = 0; m < 5; ++m) vcp8(sh + m * NT + tid, B.q + m * M + o);
+    }
+    if (any) {
+      const long long o = pcol + (long long)(k + NG) * s2;
+#pragma unroll
+      for (int m = 0; m < 9; ++m) vcp8(smt + m * NT + tid, B.khat + m * M + o);
+      vcp8(smt + 9 * NT + tid, B.jac + o);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  // ---- prologue: phi of my column at kb-3 .. kb+2 ----
+  double ph[7][4];
+#pragma unroll
+  for (int t = 0; t < 7; ++t)
+#pragma unroll
+    for (int f = 0; f < 4; ++f) ph[t][f] = 0.0;
+  if (col_in) {
+#pragma unroll
+    for (int t = 0; t < 6; ++t) {
+      const long long o = pcol + (long long)(kb - 3 + t + NG) * s2;
+      phi_of(B.q[o], B.q[M + o], B.q[2 * M + o], B.q[3 * M + o], B.q[4 * M + o], gamma, ph[t]);
+    }
+  }
+  stage(kb);
+  const double mu = P.mu, kap = P.kappa, lam = -(2.0 / 3.0) * mu;
+  for (int k = kb; k < ke; ++k) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    const bool ok = k < 0 || k >= B.n[2];
+    double* const pl = sphi + (k & 1) * (4 * PR * PC);
+    // ---- newest plane of my column into the register pipeline; plane k (my own phi and my halo cell) into shared memory ----
+    if (col_in && k + 3 + NG < B.m[2])
+      phi_of(sq[tid], sq[NT + tid], sq[2 * NT + tid], sq[3 * NT + tid], sq[4 * NT + tid], gamma, ph[6]);
+#pragma unroll
+    for (int f = 0; f < 4; ++f) pl[(f * PR + ty + 3) * PC + tx + 3] = ph[3][f];
+    if (halo_in) {
+      double hf[4];
+      phi_of(sh[tid], sh[NT + tid], sh[2 * NT + tid], sh[3 * NT + tid], sh[4 * NT + tid], gamma, hf);
+#pragma unroll
+      for (int f = 0; f < 4; ++f) pl[(f * PR + hr) * PC + hc] = hf[f];
+    }
+    double kh[3][3], J = 0.0;
+    if (any) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) kh[d][c] = smt[(d * 3 + c) * NT + tid];
+      J = smt[9 * NT + tid];
+    }
+    if (k + 1 < ke) stage(k + 1);
+    __syncthreads();
+    const bool do_xi = want_xi && !ok && col_in;
+    const bool do_eta = want_eta && !ok && !oi && col_in;
+    const bool do_zeta = want_zeta && !oi && col_in;
+    if (do_xi || do_eta || do_zeta) {
+      double g[3][4];
+#pragma unroll
+      for (int f = 0; f < 4; ++f) {
+        const double* a = pl + (f * PR + ty + 3) * PC + tx + 3;
+        const double dx = vd6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
+        const double dy = vd6c(a[-3 * PC], a[-2 * PC], a[-PC], a[PC], a[2 * PC], a[3 * PC]);
+        const double dz = vd6c(ph[0][f], ph[1][f], ph[2][f], ph[4][f], ph[5][f], ph[6][f]);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) g[c][f] = J * ((kh[0][c] * dx + kh[1][c] * dy) + kh[2][c] * dz);
+      }
+      const double u = ph[3][0], v = ph[3][1], w = ph[3][2];
+      const double div = g[0][0] + g[1][1] + g[2][2];
+      const double txx = lam * div + 2.0 * mu * g[0][0];
+      const double tyy = lam * div + 2.0 * mu * g[1][1];
+      const double tzz = lam * div + 2.0 * mu * g[2][2];
+      const double txy = mu * (g[1][0] + g[0][1]);
+      const double txz = mu * (g[2][0] + g[0][2]);
+      const double tyz = mu * (g[2][1] + g[1][2]);
+      const double bx = u * txx + v * txy + w * txz + kap * g[0][3];
+      const double by = u * txy + v * tyy + w * tyz + kap * g[1][3];
+      const double bz = u * txz + v * tyz + w * tzz + kap * g[2][3];
+      const long long p = pcol + (long long)(k + NG) * s2;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        if ((d == 0 && !do_xi) || (d == 1 && !do_eta) || (d == 2 && !do_zeta)) continue;
+        const double a = kh[d][0], b = kh[d][1], c = kh[d][2];
+        const double w0 = a * txx + b * txy + c * txz;
+        const double w1 = a * txy + b * tyy + c * tyz;
+        const double w2 = a * txz + b * tyz + c * tzz;
+        const double w3 = a * bx + b * by + c * bz;
+        if (d == 0) {
+          swx[(0 * VY + ty) * VX + tx] = w0; swx[(1 * VY + ty) * VX + tx] = w1;
+          swx[(2 * VY + ty) * VX + tx] = w2; swx[(3 * VY + ty) * VX + tx] = w3;
+        } else {
+          W[(d * 4 + 0) * M + p] = w0; W[(d * 4 + 1) * M + p] = w1;
+          W[(d * 4 + 2) * M + p] = w2; W[(d * 4 + 3) * M + p] = w3;
+        }
+      }
+    }
+    __syncthreads();
+    if (own && !oj && !ok && col_in) {
+      const long long p = pcol + (long long)(k + NG) * s2;
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        const double* a = swx + (m * VY + ty) * VX + tx;
+        W[(long long)m * M + p] = vd6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < 6; ++t)
+#pragma unroll
+      for (int f = 0; f < 4; ++f) ph[t][f] = ph[t + 1][f];
+  }
+}
+
+}  // namespace
+
+int visc_march_init() {
+  return cudaFuncSetAttribute(k_visc_march, cudaFuncAttributeMaxDynamicSharedMemorySize, VM_SMEM) == cudaSuccess ? 0 : -1;
+}
+
+// S3 point fluxes of block B (default plan): S, Fv^eta rows, Fv^zeta rows into the workspace.
+int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
+  const int ntile = (B.n[0] + 57) / 58;
+  const int TI = (B.n[0] + ntile - 1) / ntile;
+  const int nk = B.n[2] + 6;
+  // k segments: each repeats 6 planes of priming; enough CTAs for the 148 SMs (one 512-thread CTA per SM)
+  const int cols = ntile * ((B.n[1] + 6 + VY - 1) / VY);
+  int nseg = (148 * 4 + cols - 1) / cols;
+  const int maxseg = nk / 24 > 0 ? nk / 24 : 1;
+  if (nseg > maxseg) nseg = maxseg;
+  if (nseg < 1) nseg = 1;
+  const int KS = (nk + nseg - 1) / nseg;
+  dim3 grid(ntile, (B.n[1] + 6 + VY - 1) / VY, (nk + KS - 1) / KS);
+  k_visc_march<<<grid, dim3(VX, VY), VM_SMEM, c->stream>>>(B, c->pd, c->ws, TI, KS);
+  c->launches++;
+  return 0;
+}

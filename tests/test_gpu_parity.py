@@ -126,7 +126,7 @@ def test_rhs_parity(po, W, B, which):
     assert_rhs_parity(o, g, case)
 
 
-@pytest.mark.parametrize("plan", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("plan", [1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("which", ["ragged-ns", "ragged-euler", "multiblock-ns", "cylinder-ns", "tiny"])
 def test_rhs_parity_other_sweep_plans(po, W, B, which, plan):
     """cfd_set_sweep_plan: all-tiled (1), all k_march (2), xi tiled + marching (3) and the default plan with the
