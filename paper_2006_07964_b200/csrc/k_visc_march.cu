@@ -14,6 +14,7 @@
 // W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).  Same arithmetic per point as k_phi + k_visc_flux.
 #include "cfd_internal.cuh"
 #include "fastmath.cuh"
+#include <cmath>
 
 namespace {
 
@@ -23,7 +24,7 @@ constexpr int PR = VY + 6;              // plane rows j0-3 .. j0+10
 constexpr int NHALO = 2 * 3 * VX + 2 * 3 * VY;  // halo cells of the plane: 432
 constexpr int NT = VX * VY;
 // shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [4][VY][VX] | Q stage [5][NT] | halo stage [5][NT] | metric stage [10][NT]
-constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 4 * NT, SM_Q = 5 * NT, SM_H = 5 * NT, SM_M = 10 * NT;
+constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 2 * 4 * NT, SM_Q = 5 * NT, SM_H = 5 * NT, SM_M = 10 * NT;
 constexpr int VM_SMEM = (SM_PHI + SM_WX + SM_Q + SM_H + SM_M) * 8;
 
 __device__ __forceinline__ void vcp8(double* dst, const double* src) {
@@ -44,7 +45,7 @@ __device__ __forceinline__ void phi_of(double r, double m1, double m2, double m3
 __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, double* __restrict__ W, int TI, int KS) {
   extern __shared__ double vsm[];
   double* const sphi = vsm;               // [2][4][PR][PC]
-  double* const swx = sphi + SM_PHI;      // [4][VY][VX]
+  double* const swx = sphi + SM_PHI;      // [2][4][VY][VX]
   double* const sq = swx + SM_WX;         // [5][NT]
   double* const sh = sq + SM_Q;           // [5][NT]
   double* const smt = sh + SM_H;          // [10][NT]
@@ -108,6 +109,17 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
   }
   stage(kb);
   const double mu = P.mu, kap = P.kappa, lam = -(2.0 / 3.0) * mu;
+  auto s_of_plane = [&](int kk) {
+    if (own && !oj && col_in && kk >= 0 && kk < B.n[2]) {
+      const long long p = pcol + (long long)(kk + NG) * s2;
+      const double* const sx = swx + (kk & 1) * (4 * NT);
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        const double* a = sx + (m * VY + ty) * VX + tx;
+        W[(long long)m * M + p] = vd6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
+      }
+    }
+  };
   for (int k = kb; k < ke; ++k) {
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     const bool ok = k < 0 || k >= B.n[2];
@@ -133,6 +145,8 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
     }
     if (k + 1 < ke) stage(k + 1);
     __syncthreads();
+    // S = d(Fv^xi)/d(xi) of the PREVIOUS plane: its xi rows were written before this barrier (one barrier per step)
+    if (k > kb) s_of_plane(k - 1);
     const bool do_xi = want_xi && !ok && col_in;
     const bool do_eta = want_eta && !ok && !oi && col_in;
     const bool do_zeta = want_zeta && !oi && col_in;
@@ -168,21 +182,13 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
         const double w2 = a * txz + b * tyz + c * tzz;
         const double w3 = a * bx + b * by + c * bz;
         if (d == 0) {
-          swx[(0 * VY + ty) * VX + tx] = w0; swx[(1 * VY + ty) * VX + tx] = w1;
-          swx[(2 * VY + ty) * VX + tx] = w2; swx[(3 * VY + ty) * VX + tx] = w3;
+          double* const sx = swx + (k & 1) * (4 * NT);
+          sx[(0 * VY + ty) * VX + tx] = w0; sx[(1 * VY + ty) * VX + tx] = w1;
+          sx[(2 * VY + ty) * VX + tx] = w2; sx[(3 * VY + ty) * VX + tx] = w3;
         } else {
           W[(d * 4 + 0) * M + p] = w0; W[(d * 4 + 1) * M + p] = w1;
           W[(d * 4 + 2) * M + p] = w2; W[(d * 4 + 3) * M + p] = w3;
         }
-      }
-    }
-    __syncthreads();
-    if (own && !oj && !ok && col_in) {
-      const long long p = pcol + (long long)(k + NG) * s2;
-#pragma unroll
-      for (int m = 0; m < 4; ++m) {
-        const double* a = swx + (m * VY + ty) * VX + tx;
-        W[(long long)m * M + p] = vd6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
       }
     }
 #pragma unroll
@@ -190,6 +196,8 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
 #pragma unroll
       for (int f = 0; f < 4; ++f) ph[t][f] = ph[t + 1][f];
   }
+  __syncthreads();
+  s_of_plane(ke - 1);
 }
 
 }  // namespace
@@ -205,10 +213,18 @@ int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
   const int nk = B.n[2] + 6;
   // k segments: each repeats 6 planes of priming; enough CTAs for the 148 SMs (one 512-thread CTA per SM)
   const int cols = ntile * ((B.n[1] + 6 + VY - 1) / VY);
-  int nseg = (148 * 4 + cols - 1) / cols;
-  const int maxseg = nk / 24 > 0 ? nk / 24 : 1;
-  if (nseg > maxseg) nseg = maxseg;
-  if (nseg < 1) nseg = 1;
+  // whole waves of 148 CTAs (one 512-thread CTA per SM) against the 6 priming planes every segment repeats
+  int nseg = 1;
+  {
+    const int maxseg = nk / 24 > 0 ? nk / 24 : 1;
+    double best = -1.0;
+    for (int ns = 1; ns <= maxseg; ++ns) {
+      const int ks = (nk + ns - 1) / ns, n2 = (nk + ks - 1) / ks;
+      const double waves = (double)cols * n2 / 148.0;
+      const double eff = waves / ceil(waves) * ks / (ks + 3.0);
+      if (eff > best + 1e-9) { best = eff; nseg = ns; }
+    }
+  }
   const int KS = (nk + nseg - 1) / nseg;
   dim3 grid(ntile, (B.n[1] + 6 + VY - 1) / VY, (nk + KS - 1) / KS);
   k_visc_march<<<grid, dim3(VX, VY), VM_SMEM, c->stream>>>(B, c->pd, c->ws, TI, KS);
