@@ -239,6 +239,23 @@ def dominant_roofline(prof, case, n_steps, hbm_gbs, hbm_src, dfma_probe_tflops, 
     }
 
 
+def max_over_ranks(ms, dist=None, device="cpu"):
+    """Device time of the slowest rank (the job's time): all-reduce MAX over the process group, or ms itself at N=1.
+    Works on any backend (nccl on the GPUs; the CPU tests drive it with gloo, world_size 2)."""
+    if dist is None:
+        return float(ms)
+    import torch
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(points_per_rank, steps, world, ms):
+    """Whole-job Gpts/s per RK stage: every rank ran the same workload (replicas, weak scaling), 3 stages per step."""
+    return world * points_per_rank * 3 * steps / (ms * 1e-3) / 1e9
+
+
 def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, plan=0):
     import torch
 
@@ -284,10 +301,7 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, 
     if profile:
         ctx.profile_enable(False)
     launches = ctx.launch_count - l0
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, device)
     out = dict(case=case, ms=ms, pts=pts, launches=launches, prof=prof, clocks=clocks, finite=None)
 
     # sanity: the state must still be finite (a blown-up run would time garbage)
@@ -308,10 +322,7 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, 
         barrier()
         wall = (time.perf_counter() - t0) * 1e3
         ems = max(e0.elapsed_time(e1), 0.0)
-        if dist is not None:
-            t = torch.tensor([ems], dtype=torch.float64, device=device)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
+        ems = max_over_ranks(ems, dist, device)
         nbytes = sum(q.numel() * 8 for q in qh)
         out["e2e"] = dict(ms=ems, wall_ms=wall, h2d=nbytes, d2h=nbytes,
                           finite=bool(all(torch.isfinite(q).all().item() for q in qh)))
@@ -348,9 +359,9 @@ def run_ours(args):
     case, pts = main["case"], main["pts"]
     visc = int(case.params["viscous"])
     n_stage = 3 * args.steps
-    value = world * pts * n_stage / (main["ms"] * 1e-3) / 1e9
+    value = job_value(pts, args.steps, world, main["ms"])
     e2e = main["e2e"]
-    e2e_value = world * pts * n_stage / (e2e["ms"] * 1e-3) / 1e9
+    e2e_value = job_value(pts, args.steps, world, e2e["ms"])
     flop_stage = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"]
     per_gpu = value / world
     t_alu = flop_stage / (FP64_PEAK_NOMINAL_TFLOPS * 1e12)

@@ -1,21 +1,23 @@
-// S2 along xi as a marching sweep fed by TMA (cp.async.bulk.tensor, sm_100a), fp64.
+// S2 along xi as a marching sweep out of a per-warp CHUNK RING in shared memory (sm_100a, fp64).
 // P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.  Shares no code with oracle/.
 //
 // Marching along i puts the 32 lanes of a warp on 32 neighbouring j lines (stride m0 doubles), so per-lane loads would
-// use 8 bytes of every 32-byte sector.  Here each warp owns a ring of three CHUNKS in shared memory; a chunk is a TMA
-// box of 4 consecutive i positions (one aligned 32-byte sector per line) x 32 lines x all variables: one
-// cp.async.bulk.tensor for Q (5 variables) and one for khat^xi (3) per chunk, issued by one lane, completion on a
-// warp-private mbarrier.  The box lands densely ([var][line][4 positions], 32 B per line) with the hardware's 32-byte
-// swizzle (bit 4 ^= bit 7), so that the 16-byte reads "my line, positions (2h, 2h+1)" of a quarter warp hit 8 distinct
-// bank groups: conflict-free LDS.128.  Nothing crosses warps: __syncwarp and mbarriers only.
+// use 8 bytes of every 32-byte sector.  Here each warp owns a ring of three chunks; a chunk is 4 consecutive i positions
+// (one aligned 32-byte sector per line) x 32 lines x 8 variables (Q and khat^xi), laid out densely
+// ([var][line][4 positions], 32 B per line) with a 32-byte XOR swizzle (address bit 4 ^= bit 7), so that the 16-byte
+// reads "my line, positions (2h, 2h+1)" of a quarter warp hit 8 distinct bank groups: conflict-free LDS.128.
+// Nothing crosses warps: __syncwarp (and warp-private mbarriers in the TMA variant) only.
 //   * step j reads Q at j-2..j+2 and khat at j-3..j+2 as 3-4 position pairs and computes exactly what k_march does;
 //   * the output of step j (r at position j-1) is parked in the Q words of position j-3 (dead: Q is read at j-2..j+2
-//     only), i.e. r positions 4g-4..4g-1 fill exactly one chunk; when that chunk's last park is done the lanes add the
-//     viscous term S = d(Fv^xi)/d(xi) (k_visc_flux<true>, TMA-loaded into a fourth buffer) and ONE TMA store writes the
-//     box to r; the freed slot is then refilled with the chunk two ahead.
+//     only), i.e. r positions 4g-4..4g-1 fill exactly one chunk; when that chunk's last park is done it is written to r
+//     in full sectors and the freed slot is refilled with the chunk two ahead.
+// Two ways to fill the ring and to write r:
+//   k_xi_ldg (default)  warp-cooperative 16-byte cp.async (lane -> line l/2 + 16t, half l%2), swizzle by hand, STG.128;
+//   k_xi_tma (plan 5)   cp.async.bulk.tensor boxes 4 x 32 x 1 x nvar with SWIZZLE_32B, TMA store; correct, but the TMA
+//                       unit needs ~5 cycles per 32-byte box row on B200, which makes this variant TMA-bound.
 // Array index along i: a = position + NG; chunks are a/4, so r groups are aligned for NG = 6 ((NG-2) % 4 == 0) when
-// segments start at multiples of 4.  S is stored by k_visc_flux<true> two positions to the left (at a-2) so that its
-// chunks coincide with the parked chunks.
+// segments start at multiples of 4.  The xi sweep runs first (r = X); the viscous xi term S is added by the eta sweep.
+// (The VISC template parameter / the S buffer of the ring are the earlier variant in which the flush added S; unused.)
 #include <cuda.h>
 
 #include "cfd_internal.cuh"
