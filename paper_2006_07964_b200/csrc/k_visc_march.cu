@@ -7,8 +7,9 @@
 //   * the zeta stencil lives in REGISTERS: each thread keeps phi of its own column at k-3 .. k+3 (28 doubles);
 //   * the (i, j) plane of phi at k (tile + halo of 3 in j, 6 in i) lives in SHARED memory, double buffered: the xi and
 //     eta stencils read it with LDS;
-//   * Q of plane k+4, the halo cells of plane k+1 and the ten metric values of plane k+1 arrive by cp.async in
-//     thread-private shared-memory slots one step ahead (no registers held across a step);
+//   * Q of plane k+4 and the halo cells of plane k+1 arrive by cp.async in thread-private shared-memory slots one step
+//     ahead (no registers held across a step); the ten metric values are loaded before the plane barrier and used
+//     after it (staging them through shared memory as well cost more shared-memory instructions than it hid latency);
 //   * the xi rows of the flux go to shared memory and come back as S = d(Fv^xi)/d(xi), as in k_visc_flux<true>.
 // Output (workspace rows): W[0..3] = S on interior points; W[4..7] = Fv^eta rows 2..5 on (i, k) interior, j in [-3, nj+3);
 // W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).  Same arithmetic per point as k_phi + k_visc_flux.
@@ -23,9 +24,9 @@ constexpr int PC = VX + 6 + 2;          // plane columns i0-6 .. i0+63 (70), pad
 constexpr int PR = VY + 6;              // plane rows j0-3 .. j0+10
 constexpr int NHALO = 2 * 3 * VX + 2 * 3 * VY;  // halo cells of the plane: 432
 constexpr int NT = VX * VY;
-// shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [4][VY][VX] | Q stage [5][NT] | halo stage [5][NT] | metric stage [10][NT]
-constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 2 * 4 * NT, SM_Q = 5 * NT, SM_H = 5 * NT, SM_M = 10 * NT;
-constexpr int VM_SMEM = (SM_PHI + SM_WX + SM_Q + SM_H + SM_M) * 8;
+// shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [2][4][VY][VX] | Q stage [5][NT] | halo stage [5][NT]
+constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 2 * 4 * NT, SM_Q = 5 * NT, SM_H = 5 * NT;
+constexpr int VM_SMEM = (SM_PHI + SM_WX + SM_Q + SM_H) * 8;
 
 __device__ __forceinline__ void vcp8(double* dst, const double* src) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
@@ -48,7 +49,6 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
   double* const swx = sphi + SM_PHI;      // [2][4][VY][VX]
   double* const sq = swx + SM_WX;         // [5][NT]
   double* const sh = sq + SM_Q;           // [5][NT]
-  double* const smt = sh + SM_H;          // [10][NT]
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * VX + tx;
   const int i0 = blockIdx.x * TI, j0 = -3 + (int)blockIdx.y * VY;
   const int kb = -3 + (int)blockIdx.z * KS, ke = min(kb + KS, B.n[2] + 3);
@@ -84,12 +84,6 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
       const long long o = phal + (long long)(k + NG) * s2;
 #pragma unroll
       for (int m = 0; m < 5; ++m) vcp8(sh + m * NT + tid, B.q + m * M + o);
-    }
-    if (any) {
-      const long long o = pcol + (long long)(k + NG) * s2;
-#pragma unroll
-      for (int m = 0; m < 9; ++m) vcp8(smt + m * NT + tid, B.khat + m * M + o);
-      vcp8(smt + 9 * NT + tid, B.jac + o);
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
@@ -137,11 +131,12 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
     }
     double kh[3][3], J = 0.0;
     if (any) {
+      const long long o = pcol + (long long)(k + NG) * s2;
 #pragma unroll
       for (int d = 0; d < 3; ++d)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) kh[d][c] = smt[(d * 3 + c) * NT + tid];
-      J = smt[9 * NT + tid];
+        for (int c = 0; c < 3; ++c) kh[d][c] = __ldg(B.khat + (d * 3 + c) * M + o);
+      J = __ldg(B.jac + o);
     }
     if (k + 1 < ke) stage(k + 1);
     __syncthreads();
