@@ -47,8 +47,8 @@ HBM_FALLBACK_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
 # `ncu --set full` capture (profiles/), keyed by (workload, kernel class); None until captured.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1_marching.md: k_xi_ldg<0> at 256^3, 2.034 GB read + 1.014 GB written per launch
-    ("sweep256", "inviscid_xi"): 3.048e9,
+    # profiles/r1_marching.md: k_xi_ldg<0> at 256^3, 2.038 GB read + 1.017 GB written per launch
+    ("sweep256", "inviscid_xi"): 3.055e9,
 }
 
 WORKLOADS = {
