@@ -350,6 +350,44 @@ def test_full_size_sampled_parity(po, W, B, which):
             subbox_check(po, g, case, b, lo, ext, S)
 
 
+@pytest.mark.parametrize("which", ["C4-8x96", "sweep-256"])
+def test_full_size_fused_stage_sampled(po, W, B, which):
+    """cfd_stage_fused at full size, in the launch configuration bench.py times: around sampled points the oracle
+    recomputes R from the GPU's own state before the stage (sub-box with its ghosts); the GPU's state after stage 1 must
+    equal Q + dt R there (Eq. 20), and Q^n must be the old state bit for bit."""
+    import torch
+
+    case = {"C4-8x96": lambda: W.c4_multiblock(96), "sweep-256": lambda: W.sweep_block(256)}[which]()
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    g.step(case.dt)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(4321)
+    b = len(case.dims) - 1
+    n = case.dims[b]
+    boxes, ext = sample_boxes(n, rng, count=4)
+    saved = []
+    for lo in boxes:
+        sl = tuple(slice(lo[a], lo[a] + ext[a] + 2 * NG) for a in (2, 1, 0))
+        saved.append({name: g.field(b, name)[(slice(None),) + sl].cpu().numpy().copy() for name in ("q", "khat", "jac")})
+    g.stage_fused(1, case.dt)
+    torch.cuda.synchronize()
+    for lo, sv in zip(boxes, saved):
+        o = po.Oracle([tuple(ext)], [], case.params)
+        for name in ("q", "khat", "jac"):
+            o.field(0, name)[...] = sv[name]
+        o.rhs()
+        isl = tuple(slice(lo[a] + NG, lo[a] + NG + ext[a]) for a in (2, 1, 0))
+        q_old = o.interior(0, "q")
+        expect = q_old + case.dt * o.interior(0, "r")
+        got = g.field(b, "q")[(slice(None),) + isl].cpu().numpy()
+        qn = g.field(b, "qn")[(slice(None),) + isl].cpu().numpy()
+        scale = np.abs(q_old).max()  # the field's max magnitude (w ~ 0 in the TGV field: no per-component scale)
+        err = np.abs(got - expect).max(axis=(1, 2, 3)) / scale
+        assert err.max() < 1e-12, (which, lo, err)
+        assert np.array_equal(qn, q_old)
+
+
 # ------------------------------------------------------------------------------------------------
 # error behaviour through the ABI
 # ------------------------------------------------------------------------------------------------
