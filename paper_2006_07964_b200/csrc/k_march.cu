@@ -158,6 +158,7 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
       }
     }
     double ULc[5] = {0, 0, 0, 0, 0}, Phip[5] = {0, 0, 0, 0, 0};
+#pragma unroll 2
     for (int j = p0 - 1; j <= p1; ++j) {
       // ---- prefetch for the next step: Q, khat, W of position j+3; operands of the output at position j ----
       if (j < p1) {
