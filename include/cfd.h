@@ -85,9 +85,10 @@ typedef struct {
   double* jac;  /* [1][M] J (Eq. 8) */
 } cfd_block_ptrs;
 
-/* Bytes of device scratch the caller must pass to cfd_create_blocks (16 doubles per point of the
- * largest block: 12 viscous point-flux rows + phi = (u,v,w,T), or the 9 metric first derivatives; plus
- * reduction partials). */
+/* Bytes of device scratch the caller must pass to cfd_create_blocks: 16 doubles per stored point of EVERY block
+ * (each block has its own area, so that the per-block kernels of a multi-block case can run concurrently: the
+ * viscous rows S, Fv^eta, Fv^zeta; phi = (u,v,w,T) for the tiled plans; the 9 metric first derivatives during
+ * cfd_compute_metrics), plus the partial sums of the residual reduction. */
 size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params* params);
 
 /* Build a context over nblocks point-matched blocks (a patch is a whole block face).

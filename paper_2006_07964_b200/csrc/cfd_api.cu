@@ -9,16 +9,13 @@ static thread_local std::string g_create_err;
 
 static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD_FACE_INTERFACE; }
 
-size_t ws_partials_offset_doubles(long long max_M) { return (size_t)16 * (size_t)max_M; }
+size_t ws_partials_offset_doubles(const cfd_ctx* c) { return (size_t)16 * (size_t)c->sum_M; }
 int rk_max_partial_blocks() { return 16384; }
 
 extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
-  long long mx = 0;
-  for (int b = 0; b < nblocks; ++b) {
-    long long M = (long long)(dims[b].ni + 2 * NG) * (dims[b].nj + 2 * NG) * (dims[b].nk + 2 * NG);
-    if (M > mx) mx = M;
-  }
-  return (ws_partials_offset_doubles(mx) + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
+  long long sum = 0;  // every block has its own 16 M doubles (the blocks' kernels run concurrently on side streams)
+  for (int b = 0; b < nblocks; ++b) sum += (long long)(dims[b].ni + 2 * NG) * (dims[b].nj + 2 * NG) * (dims[b].nk + 2 * NG);
+  return ((size_t)16 * (size_t)sum + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
 }
 
 // the six assignments of three buffers to the roles (q, qn, r): id -> role[]
@@ -136,6 +133,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
     for (int t = 0; t < 6; ++t)
       if (!pp[t] || ((uintptr_t)pp[t] & 15u)) { delete c; return fail_create(CFD_E_ARG, "cfd_create_blocks: null or misaligned (16 B) field pointer"); }
     if (B.M > c->max_M) c->max_M = B.M;
+    c->sum_M += B.M;
   }
   // ---- faces ----
   c->faces.assign(faces, faces + nfaces);
@@ -175,6 +173,10 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   }
   c->ws = (double*)workspace;
   c->ws_bytes = workspace_bytes;
+  {
+    long long off = 0;
+    for (BlockDev& B : c->blk) { B.ws = c->ws + 16 * off; off += B.M; }
+  }
   plan_copies(c);
   // ---- small device-side descriptor arrays (a few KB; the only allocations the library makes) ----
   auto cuda_fail = [&](cudaError_t e, const char* what) {
@@ -202,6 +204,13 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   }
   set_roles(c, 0, 1, 2);
   xi_tma_setup(c);
+  if (nblocks > 1) {
+    for (int t = 0; t < cfd_ctx::NSIDE; ++t) {
+      if ((e = cudaStreamCreateWithFlags(&c->side[t], cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
+      if ((e = cudaEventCreateWithFlags(&c->ev_join[t], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+    }
+    if ((e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+  }
   for (int p = 1; p <= 3; ++p) {
     if (c->tasks[p].empty()) continue;
     if ((e = cudaMalloc(&c->d_tasks[p], sizeof(CopyTask) * c->tasks[p].size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc tasks");
@@ -219,6 +228,11 @@ extern "C" int cfd_destroy(cfd_ctx* c) {
   if (!c) return CFD_OK;
   if (c->d_blocks_all) cudaFree(c->d_blocks_all);
   xi_tma_free(c);
+  for (int t = 0; t < cfd_ctx::NSIDE; ++t) {
+    if (c->side[t]) cudaStreamDestroy(c->side[t]);
+    if (c->ev_join[t]) cudaEventDestroy(c->ev_join[t]);
+  }
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   for (int p = 1; p <= 3; ++p)
     if (c->d_tasks[p]) cudaFree(c->d_tasks[p]);
   if (c->d_flag) cudaFree(c->d_flag);

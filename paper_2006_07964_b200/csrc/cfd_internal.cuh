@@ -18,6 +18,7 @@ struct BlockDev {
   long long M;
   long long s[3];
   double *q, *qn, *r, *xyz, *khat, *jac;
+  double* ws;  // this block's 16 M doubles of scratch inside the caller's workspace (viscous rows, phi / metric derivatives)
   // offset of interior node (0,0,0)
   __host__ __device__ inline long long idx(int i, int j, int k) const {
     return ((long long)(k + NG) * m[1] + (j + NG)) * m[0] + (i + NG);
@@ -64,6 +65,10 @@ struct cfd_ctx {
   double* ws = nullptr;
   size_t ws_bytes = 0;
   long long max_M = 0;
+  long long sum_M = 0;                // sum of M over the blocks: the per-block scratch areas are 16 M doubles each
+  static constexpr int NSIDE = 4;     // side streams: the blocks of a multi-block case run their per-block kernels concurrently
+  cudaStream_t side[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
   long long launches = 0;
   int sweep_plan = 0;                 // cfd_set_sweep_plan
   bool visc_tiled = false;            // cfd_set_sweep_plan(6): plan 0 with k_phi + k_visc_flux instead of k_visc_march
@@ -129,7 +134,7 @@ bool xi_tma_ok(const cfd_ctx* c, int b);
 bool xi_ldg_ok(const cfd_ctx* c, int b);
 int launch_xi_tma(cfd_ctx* c, int b, bool tma);
 
-size_t ws_partials_offset_doubles(long long max_M);
+size_t ws_partials_offset_doubles(const cfd_ctx* c);
 int rk_max_partial_blocks();
 
 #define CUDA_TRY(ctx, expr)                                                      \

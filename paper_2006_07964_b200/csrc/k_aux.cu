@@ -259,9 +259,9 @@ __global__ void __launch_bounds__(256) k_metric_khat(BlockDev B, const double* _
 int launch_metrics(cfd_ctx* c) {
   for (const BlockDev& B : c->blk) {
     ProfScope ps(c, PK_METRICS);
-    k_metric_d1<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, c->ws);
+    k_metric_d1<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, B.ws);
     const long long box = (long long)(B.n[0] + 6) * (B.n[1] + 6) * (B.n[2] + 6);
-    k_metric_khat<<<(unsigned)((box + 255) / 256), 256, 0, c->stream>>>(B, c->ws, c->d_flag);
+    k_metric_khat<<<(unsigned)((box + 255) / 256), 256, 0, c->stream>>>(B, B.ws, c->d_flag);
     c->launches += 2;
   }
   CUDA_TRY(c, cudaGetLastError());
@@ -329,7 +329,7 @@ __global__ void k_res_final(const double* __restrict__ partials, int n, double* 
 int launch_rk(cfd_ctx* c, int stage, double dt) {
   const double a = stage == 1 ? 0.0 : (stage == 2 ? 3.0 / 4.0 : 1.0 / 3.0);
   const double b = stage == 1 ? 1.0 : (stage == 2 ? 1.0 / 4.0 : 2.0 / 3.0);
-  double* partials = c->ws + ws_partials_offset_doubles(c->max_M);
+  double* partials = c->ws + ws_partials_offset_doubles(c);
   int used = 0;
   for (const BlockDev& B : c->blk) {
     const long long N = (long long)B.n[0] * B.n[1] * B.n[2];

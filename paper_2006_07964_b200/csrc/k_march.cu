@@ -514,10 +514,10 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
   MarchArgs A;
   A.q = B.q + o0;
   A.kh = B.khat + (long long)(dir * 3) * B.M + o0;
-  A.W = visc ? c->ws + (long long)(dir * 4) * B.M + o0 : nullptr;
+  A.W = visc ? B.ws + (long long)(dir * 4) * B.M + o0 : nullptr;
   A.jac = B.jac + o0;
   A.qn = B.qn + o0;
-  A.Sx = c->ws + o0;
+  A.Sx = B.ws + o0;
   A.r = B.r + o0;
   A.partials = rk ? rk->partials : nullptr;
   A.dt = rk ? rk->dt : 0.0; A.rk_a = rk ? rk->a : 0.0; A.rk_b = rk ? rk->b : 0.0;
@@ -560,7 +560,7 @@ int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
   A.q = B.q + o0;
   A.kh = B.khat + o0;
   A.W = nullptr;
-  A.Sx = visc ? c->ws + o0 : nullptr;
+  A.Sx = visc ? B.ws + o0 : nullptr;
   A.jac = B.jac + o0;
   A.r = B.r + o0;
   A.M = B.M;

@@ -136,15 +136,26 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
   rk.dt = dt;
   rk.a = fused_stage == 2 ? 3.0 / 4.0 : (fused_stage == 3 ? 1.0 / 3.0 : 0.0);
   rk.b = fused_stage == 2 ? 1.0 / 4.0 : (fused_stage == 3 ? 2.0 / 3.0 : 1.0);
-  double* const partials = c->ws + ws_partials_offset_doubles(c->max_M);
+  double* const partials = c->ws + ws_partials_offset_doubles(c);
   const long long cap = (long long)rk_max_partial_blocks() * (long long)c->blk.size();
   long long used = 0;
+  // Blocks are independent until the ghost fill: with several blocks (and no per-kernel timing) each block's chain of
+  // kernels goes to one of the side streams, forked from and joined back into the context's stream, so that small
+  // blocks (C4: 8 x 96^3, about one wave of CTAs per kernel) fill the GPU together.  Every block has its own scratch.
+  cudaStream_t const main_stream = c->stream;
+  const bool fork = c->blk.size() > 1 && !c->prof_on && c->side[0] != nullptr;
+  if (fork) {
+    CUDA_TRY(c, cudaEventRecord(c->ev_fork, main_stream));
+    for (int t = 0; t < cfd_ctx::NSIDE; ++t) CUDA_TRY(c, cudaStreamWaitEvent(c->side[t], c->ev_fork, 0));
+  }
+  int bi = 0;
   for (const BlockDev& B : c->blk) {
+    if (fork) c->stream = c->side[bi++ % cfd_ctx::NSIDE];
     if (c->pd.viscous && c->sweep_plan == 0 && !c->visc_tiled) {
       ProfScope ps(c, PK_VISC_FLUX);
       launch_visc_march(c, B);
     } else if (c->pd.viscous) {
-      double* phi = c->ws + 12 * c->max_M;
+      double* phi = B.ws + 12 * B.M;
       { ProfScope ps(c, PK_VISC_PHI); k_phi<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, c->pd.gamma, phi); }
       const bool sxi = c->sweep_plan == 0;
       int T, threads;
@@ -152,8 +163,8 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
       visc_geometry(B, sxi, &T, &g1, &threads);
       {
         ProfScope ps(c, PK_VISC_FLUX);
-        if (sxi) k_visc_flux<true><<<g1, threads, 0, c->stream>>>(B, c->pd, phi, c->ws, T);
-        else k_visc_flux<false><<<g1, threads, 0, c->stream>>>(B, c->pd, phi, c->ws, T);
+        if (sxi) k_visc_flux<true><<<g1, threads, 0, c->stream>>>(B, c->pd, phi, B.ws, T);
+        else k_visc_flux<false><<<g1, threads, 0, c->stream>>>(B, c->pd, phi, B.ws, T);
       }
       c->launches += 2;
     }
@@ -161,8 +172,15 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
     rk.max_ctas = cap - used < rk_max_partial_blocks() ? cap - used : rk_max_partial_blocks();
     int ctas = 0;
     const int rc = launch_sweeps(c, B, fused_stage ? &rk : nullptr, &ctas);
-    if (rc != 0) return rc;
+    if (rc != 0) { c->stream = main_stream; return rc; }
     if (fused_stage == 1) used += ctas;
+  }
+  c->stream = main_stream;
+  if (fork) {
+    for (int t = 0; t < cfd_ctx::NSIDE; ++t) {
+      CUDA_TRY(c, cudaEventRecord(c->ev_join[t], c->side[t]));
+      CUDA_TRY(c, cudaStreamWaitEvent(main_stream, c->ev_join[t], 0));
+    }
   }
   if (fused_stage == 1) {
     ProfScope ps(c, PK_RES);

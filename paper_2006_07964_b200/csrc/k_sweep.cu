@@ -228,8 +228,8 @@ void launch_one(cfd_ctx* c, const BlockDev& B, bool visc) {
   else if (DIR == 1) { grid = dim3((B.n[0] + NL - 1) / NL, (B.n[1] + T - 1) / T, B.n[2]); block = dim3(NL, TS); }
   else { grid = dim3((B.n[0] + NL - 1) / NL, B.n[1], (B.n[2] + T - 1) / T); block = dim3(NL, TS); }
   const size_t sm = SweepCfg<DIR>::smem_doubles(visc) * sizeof(double);
-  if (visc) k_sweep<DIR, ACC, true><<<grid, block, sm, c->stream>>>(B, c->pd, c->ws);
-  else k_sweep<DIR, ACC, false><<<grid, block, sm, c->stream>>>(B, c->pd, c->ws);
+  if (visc) k_sweep<DIR, ACC, true><<<grid, block, sm, c->stream>>>(B, c->pd, B.ws);
+  else k_sweep<DIR, ACC, false><<<grid, block, sm, c->stream>>>(B, c->pd, B.ws);
 }
 
 }  // namespace

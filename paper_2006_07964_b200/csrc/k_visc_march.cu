@@ -222,7 +222,7 @@ int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
   }
   const int KS = (nk + nseg - 1) / nseg;
   dim3 grid(ntile, (B.n[1] + 6 + VY - 1) / VY, (nk + KS - 1) / KS);
-  k_visc_march<<<grid, dim3(VX, VY), VM_SMEM, c->stream>>>(B, c->pd, c->ws, TI, KS);
+  k_visc_march<<<grid, dim3(VX, VY), VM_SMEM, c->stream>>>(B, c->pd, B.ws, TI, KS);
   c->launches++;
   return 0;
 }

@@ -503,7 +503,7 @@ void xi_tma_setup(cfd_ctx* c) {
     bool ok = true;
     for (int t = 0; t < 3; ++t) ok = ok && encode(fn, &X.st[t], B, c->base[t][b], 5);
     ok = ok && encode(fn, &X.kh, B, B.khat, 3);
-    ok = ok && encode(fn, &X.sx, B, c->ws, 4);
+    ok = ok && encode(fn, &X.sx, B, B.ws, 4);
     X.ok = ok;
   }
 }
@@ -543,7 +543,7 @@ int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
   dim3 grid((unsigned)ctas, (unsigned)((A.n + A.S - 1) / A.S));
   if (!tma) {
     XiLArgs L;
-    L.q = B.q; L.kh = B.khat; L.sx = c->ws; L.r = B.r;
+    L.q = B.q; L.kh = B.khat; L.sx = B.ws; L.r = B.r;
     L.M = B.M; L.s1 = B.s[1]; L.s2 = B.s[2];
     L.g = A;
     k_xi_ldg<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);  // S is added by the eta sweep
