@@ -19,7 +19,12 @@
 // 5/6/3, decomposition/permutation equivalence and brute force (tests/test_oracle_*.py).
 // "parity unpinned" items (vs. the AUTHORS' closed code): the eigenvector scaling (U4),
 // the half-point metric interpolation (U5), ghost-layer closure (U12) and the wall /
-// far-field formulas (U13, U14), which the paper does not print.
+// far-field formulas (U13, U14), which the paper does not print.  The readings themselves
+// are pinned against mathematics in tests/test_oracle_bc_pins.py: the wall closure by
+// polynomial exactness (quartics with zero slope return a(0)), the subsonic far field by
+// its Riemann invariants and the upwind side's entropy / tangential velocity with distinct
+// interior and far-field states, cfl_dt (U16) by a hand formula on a Cartesian grid, the
+// stage-1 residual (U17) by the plain sum of squares of the R field.
 //
 // Everything is templated on the scalar type T so that oracle/flopcount.cpp can run the
 // same per-point routines with a counting type (the contract flop count).

@@ -215,14 +215,19 @@ class Oracle:
     def cfl_dt(self, cfl):
         return lib().orc_cfl_dt(self.h, cfl)
 
+    def stage(self, s, dt, want_res=False):
+        """One RK stage in the order of Fig. 2: RHS, Eq. 20, ghost fill, physical BCs."""
+        self.rhs()
+        r = self.rk_stage(s, dt, want_res=want_res)
+        self.exchange_interfaces()
+        self.apply_bc()
+        return r
+
     def step(self, dt):
         """One TVD-RK3 step in the order of Fig. 2."""
         res = None
         for s in (1, 2, 3):
-            self.rhs()
-            r = self.rk_stage(s, dt, want_res=(s == 1))
+            r = self.stage(s, dt, want_res=(s == 1))
             if s == 1:
                 res = r
-            self.exchange_interfaces()
-            self.apply_bc()
         return res
