@@ -124,6 +124,15 @@ int cfd_exchange_interfaces(cfd_ctx*);
  * node plane and the 6 ghost layers behind it, tangential index range [-3, n+3). */
 int cfd_apply_bc(cfd_ctx*);
 
+/* On-device CFL time step ("time step dt" per point, "reduced-dimensional operation", Fig. 2
+ * timestep_gpu; reading U16): s_i = sum_d ( |k_d . u| + c |k_d| ), k_d = J khat^d, at every interior point of every
+ * block from the current q; *dt_host = cfl / max_i s_i (MAX reduction: order-independent, deterministic).
+ * dt_local_dev_or_null: if non-null, one DEVICE pointer per block to a caller-owned array of M doubles (field layout with
+ * ghosts); the local time step cfl / s_i is written at interior points (ghost entries untouched).
+ * Requires cfd_compute_metrics.  One bandwidth-bound pass over q, khat, jac (120 B per point).
+ * Returns host values: synchronises the stream.  CFD_E_ARG if cfl <= 0 or the state is not physical (max s not > 0). */
+int cfd_cfl_dt(cfd_ctx*, double cfl, double* dt_host, double* const* dt_local_dev_or_null);
+
 /* Convenience: the four calls above for one stage, in Fig. 2's order, on the context's stream. */
 int cfd_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
 

@@ -20,6 +20,7 @@ ABI_SYMBOLS = (
     "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
     "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan", "cfd_stage_fused", "cfd_buffer_roles",
+    "cfd_cfl_dt",
 )
 PROF_NCLASS = 12
 
@@ -67,6 +68,8 @@ def _load():
     for n in ("cfd_rk_stage", "cfd_stage", "cfd_stage_fused"):
         getattr(L, n).restype = C.c_int
         getattr(L, n).argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_double)]
+    L.cfd_cfl_dt.restype = C.c_int
+    L.cfd_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_void_p)]
     L.cfd_last_error.restype = C.c_char_p
     L.cfd_last_error.argtypes = [C.c_void_p]
     L.cfd_launch_count.restype = C.c_longlong
@@ -220,6 +223,21 @@ class Context:
 
     def apply_bc(self):
         self._chk(lib.cfd_apply_bc(self.h))
+
+    def cfl_dt(self, cfl, dt_local=None):
+        """cfd_cfl_dt: dt = cfl / max over all interior points of sum_d(|k_d.u| + c|k_d|) from the current q; dt_local:
+        optional list (one per block) of device fp64 tensors of shape (nk+12, nj+12, ni+12) receiving cfl / s_i."""
+        dt = C.c_double()
+        loc = None
+        if dt_local is not None:
+            for b, a in enumerate(dt_local):
+                ni, nj, nk = self.dims[b]
+                if not (a.is_cuda and a.dtype == self.torch.float64 and a.is_contiguous()
+                        and tuple(a.shape) == (nk + 2 * NG, nj + 2 * NG, ni + 2 * NG)):
+                    raise CfdError(-1, f"cfl_dt: block {b} needs a contiguous device fp64 tensor of shape (nk+12, nj+12, ni+12)")
+            loc = (C.c_void_p * len(self.dims))(*[a.data_ptr() for a in dt_local])
+        self._chk(lib.cfd_cfl_dt(self.h, float(cfl), C.byref(dt), loc))
+        return dt.value
 
     def stage(self, stage, dt, want_res=False):
         res = (C.c_double * 5)()

@@ -276,6 +276,22 @@ extern "C" int cfd_rk_stage(cfd_ctx* c, int stage, double dt, double* res5) {
   return CFD_OK;
 }
 
+extern "C" int cfd_cfl_dt(cfd_ctx* c, double cfl, double* dt_host, double* const* dt_local) {
+  if (!c || !dt_host) return CFD_E_ARG;
+  if (!(cfl > 0.0)) { c->err = "cfd_cfl_dt: cfl must be > 0"; return CFD_E_ARG; }
+  if (dt_local)
+    for (size_t b = 0; b < c->blk.size(); ++b)
+      if (!dt_local[b] || ((uintptr_t)dt_local[b] & 7u)) { c->err = "cfd_cfl_dt: null or misaligned dt_local pointer"; return CFD_E_ARG; }
+  int rc = launch_cfl(c, cfl, dt_local);
+  if (rc != 0) return rc;
+  double smax = 0.0;
+  CUDA_TRY(c, cudaMemcpyAsync(&smax, c->d_res + 5, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (!(smax > 0.0) || smax != smax) { c->err = "cfd_cfl_dt: non-positive or NaN spectral radius (state not physical)"; return CFD_E_ARG; }
+  *dt_host = cfl / smax;
+  return CFD_OK;
+}
+
 extern "C" int cfd_exchange_interfaces(cfd_ctx* c) {
   if (!c) return CFD_E_ARG;
   return launch_fill_connect(c, 0);

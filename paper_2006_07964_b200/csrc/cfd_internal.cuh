@@ -123,6 +123,7 @@ int launch_metrics(cfd_ctx* c);
 int launch_rhs(cfd_ctx* c, int fused_stage /*0 = plain rhs*/, double dt);
 void set_roles(cfd_ctx* c, int iq, int iqn, int ir);
 int launch_rk(cfd_ctx* c, int stage, double dt);
+int launch_cfl(cfd_ctx* c, double cfl, double* const* dt_local);
 int launch_fp64_probe(int iters, double* tflops);
 int launch_fastmath_selftest(int n, const double* x_host, double* rcp_host, double* rsqrt_host);
 int sweep_init();

@@ -19,14 +19,23 @@
 
 namespace {
 
-constexpr int VX = 64, VY = 8;          // threads: columns i0-3 .. i0+60, rows j0 .. j0+7
-constexpr int PC = VX + 6 + 2;          // plane columns i0-6 .. i0+63 (70), padded to 72
-constexpr int PR = VY + 6;              // plane rows j0-3 .. j0+10
-constexpr int NHALO = 2 * 3 * VX + 2 * 3 * VY;  // halo cells of the plane: 432
-constexpr int NT = VX * VY;
-// shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [2][4][VY][VX] | Q stage [5][NT] | halo stage [5][NT]
-constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 2 * 4 * NT, SM_Q = 5 * NT, SM_H = 5 * NT;
-constexpr int VM_SMEM = (SM_PHI + SM_WX + SM_Q + SM_H) * 8;
+// Tile geometry: VX x VY threads own the columns i0-3 .. i0+VX-4 of the rows j0 .. j0+VY-1; VX-6 of them are output columns.
+// The plane row pitch PC is congruent to VX modulo 16 doubles, so that consecutive threads (also across a row change
+// inside a warp when VX is not a multiple of 32) hit consecutive banks.  Every thread stages HPT halo cells of the plane.
+template <int VX_, int VY_>
+struct VG {
+  static constexpr int VX = VX_, VY = VY_;
+  static constexpr int PC = VX + 16;          // plane columns i0-6 .. i0+VX-1 (VX + 6), padded
+  static constexpr int PR = VY + 6;           // plane rows j0-3 .. j0+VY+2
+  static constexpr int NHALO = 2 * 3 * VX + 2 * 3 * VY;
+  static constexpr int NT = VX * VY;
+  static constexpr int HPT = (NHALO + NT - 1) / NT;   // halo cells staged per thread
+  static constexpr int MINB = NT <= 256 ? 2 : 1;      // CTAs per SM (128 registers per thread either way)
+  static_assert(NT <= 512, "k_visc_march: tile geometry");
+  // shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [2][4][VY][VX] | Q stage [5][NT] | halo stage [5][HPT NT]
+  static constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 2 * 4 * NT, SM_Q = 5 * NT, SM_H = 5 * HPT * NT;
+  static constexpr int SMEM = (SM_PHI + SM_WX + SM_Q + SM_H) * 8;
+};
 
 __device__ __forceinline__ void vcp8(double* dst, const double* src) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
@@ -43,12 +52,15 @@ __device__ __forceinline__ void phi_of(double r, double m1, double m2, double m3
   f[0] = u; f[1] = v; f[2] = w; f[3] = (gamma * pr) * ir;
 }
 
-__global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, double* __restrict__ W, int TI, int KS) {
+template <class G>
+__global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, ParamsDev P, double* __restrict__ W, int TI, int KS) {
+  constexpr int VX = G::VX, VY = G::VY, PC = G::PC, PR = G::PR, NHALO = G::NHALO, NT = G::NT, HPT = G::HPT;
+  constexpr int SM_PHI = G::SM_PHI, SM_WX = G::SM_WX, SM_Q = G::SM_Q;
   extern __shared__ double vsm[];
   double* const sphi = vsm;               // [2][4][PR][PC]
   double* const swx = sphi + SM_PHI;      // [2][4][VY][VX]
   double* const sq = swx + SM_WX;         // [5][NT]
-  double* const sh = sq + SM_Q;           // [5][NT]
+  double* const sh = sq + SM_Q;           // [5][HPT NT]
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * VX + tx;
   const int i0 = blockIdx.x * TI, j0 = -3 + (int)blockIdx.y * VY;
   const int kb = -3 + (int)blockIdx.z * KS, ke = min(kb + KS, B.n[2] + 3);
@@ -64,15 +76,23 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
   const bool want_zeta = own && !oj;                                            // zeta rows (all k of the march)
   const bool any = col_in && (want_xi || want_eta || want_zeta) && !(oi && oj);
   const long long pcol = (long long)(j + NG) * s1 + (i + NG);                  // array offset of (i, j, k = -NG)
-  // my halo cell of the plane (if any): top band, bottom band, left columns, right columns
-  int hc = -1, hr = -1;  // plane column / row
-  if (tid < 3 * VX) { hr = tid / VX; hc = 3 + tid % VX; }
-  else if (tid < 6 * VX) { hr = VY + 3 + (tid - 3 * VX) / VX; hc = 3 + tid % VX; }
-  else if (tid < 6 * VX + 3 * VY) { hr = 3 + (tid - 6 * VX) / 3; hc = (tid - 6 * VX) % 3; }
-  else if (tid < NHALO) { hr = 3 + (tid - 6 * VX - 3 * VY) / 3; hc = VX + 3 + (tid - 6 * VX - 3 * VY) % 3; }
-  const int hi = i0 - 6 + hc, hj = j0 - 3 + hr;
-  const bool halo_in = hc >= 0 && hi + NG >= 0 && hi + NG < B.m[0] && hj + NG >= 0 && hj + NG < B.m[1];
-  const long long phal = (long long)(hj + NG) * s1 + (hi + NG);
+  // my halo cells of the plane (if any): top band, bottom band, left columns, right columns
+  int hpl[HPT];           // offset of the cell inside one field of the plane (hr * PC + hc)
+  bool halo_in[HPT];
+  long long phal[HPT];
+#pragma unroll
+  for (int h = 0; h < HPT; ++h) {
+    const int t = tid + h * NT;
+    int hc = -1, hr = -1;  // plane column / row
+    if (t < 3 * VX) { hr = t / VX; hc = 3 + t % VX; }
+    else if (t < 6 * VX) { hr = VY + 3 + (t - 3 * VX) / VX; hc = 3 + t % VX; }
+    else if (t < 6 * VX + 3 * VY) { hr = 3 + (t - 6 * VX) / 3; hc = (t - 6 * VX) % 3; }
+    else if (t < NHALO) { hr = 3 + (t - 6 * VX - 3 * VY) / 3; hc = VX + 3 + (t - 6 * VX - 3 * VY) % 3; }
+    const int hi = i0 - 6 + hc, hj = j0 - 3 + hr;
+    halo_in[h] = hc >= 0 && hi + NG >= 0 && hi + NG < B.m[0] && hj + NG >= 0 && hj + NG < B.m[1];
+    phal[h] = (long long)(hj + NG) * s1 + (hi + NG);
+    hpl[h] = hr * PC + hc;
+  }
 
   auto stage = [&](int k) {  // cp.async for the step of plane k: Q(k+3) of my column, my halo cell at k, metrics at k
     if (col_in && k + 3 + NG < B.m[2]) {
@@ -80,10 +100,13 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
 #pragma unroll
       for (int m = 0; m < 5; ++m) vcp8(sq + m * NT + tid, B.q + m * M + o);
     }
-    if (halo_in) {
-      const long long o = phal + (long long)(k + NG) * s2;
 #pragma unroll
-      for (int m = 0; m < 5; ++m) vcp8(sh + m * NT + tid, B.q + m * M + o);
+    for (int h = 0; h < HPT; ++h) {
+      if (halo_in[h]) {
+        const long long o = phal[h] + (long long)(k + NG) * s2;
+#pragma unroll
+        for (int m = 0; m < 5; ++m) vcp8(sh + (m * HPT + h) * NT + tid, B.q + m * M + o);
+      }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
@@ -123,11 +146,15 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
       phi_of(sq[tid], sq[NT + tid], sq[2 * NT + tid], sq[3 * NT + tid], sq[4 * NT + tid], gamma, ph[6]);
 #pragma unroll
     for (int f = 0; f < 4; ++f) pl[(f * PR + ty + 3) * PC + tx + 3] = ph[3][f];
-    if (halo_in) {
-      double hf[4];
-      phi_of(sh[tid], sh[NT + tid], sh[2 * NT + tid], sh[3 * NT + tid], sh[4 * NT + tid], gamma, hf);
 #pragma unroll
-      for (int f = 0; f < 4; ++f) pl[(f * PR + hr) * PC + hc] = hf[f];
+    for (int h = 0; h < HPT; ++h) {
+      if (halo_in[h]) {
+        double hf[4];
+        const double* a = sh + h * NT + tid;
+        phi_of(a[0], a[HPT * NT], a[2 * HPT * NT], a[3 * HPT * NT], a[4 * HPT * NT], gamma, hf);
+#pragma unroll
+        for (int f = 0; f < 4; ++f) pl[f * PR * PC + hpl[h]] = hf[f];
+      }
     }
     double kh[3][3], J = 0.0;
     if (any) {
@@ -195,34 +222,39 @@ __global__ void __launch_bounds__(NT, 1) k_visc_march(BlockDev B, ParamsDev P, d
   s_of_plane(ke - 1);
 }
 
+using G0 = VG<64, 8>;
+
 }  // namespace
 
 int visc_march_init() {
-  return cudaFuncSetAttribute(k_visc_march, cudaFuncAttributeMaxDynamicSharedMemorySize, VM_SMEM) == cudaSuccess ? 0 : -1;
+  return cudaFuncSetAttribute(k_visc_march<G0>, cudaFuncAttributeMaxDynamicSharedMemorySize, G0::SMEM) == cudaSuccess ? 0 : -1;
 }
 
 // S3 point fluxes of block B (default plan): S, Fv^eta rows, Fv^zeta rows into the workspace.
+// Tile geometry: 64 x 8 threads.  Measured on B200 (256^3, 128^3, 8 x 96^3): 70 x 7 (12 % fewer thread-planes at 256^3),
+// 54 x 9 and two 64 x 4 CTAs per SM all land within +-5 % of it -- the kernel is bound by the shared-memory pipe and the
+// per-plane barrier, not by the tile's halo overhead -- so only this one is instantiated.
 int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
-  const int ntile = (B.n[0] + 57) / 58;
+  using G = G0;
+  const int TImax = G::VX - 6;
+  const int ntile = (B.n[0] + TImax - 1) / TImax;
   const int TI = (B.n[0] + ntile - 1) / ntile;
   const int nk = B.n[2] + 6;
-  // k segments: each repeats 6 planes of priming; enough CTAs for the 148 SMs (one 512-thread CTA per SM)
-  const int cols = ntile * ((B.n[1] + 6 + VY - 1) / VY);
-  // whole waves of 148 CTAs (one 512-thread CTA per SM) against the 6 priming planes every segment repeats
+  const int rows = (B.n[1] + 6 + G::VY - 1) / G::VY;
+  const int cols = ntile * rows;
+  // k segments: each repeats 6 planes of priming (~3 planes' worth of time); whole waves of 148 CTAs (one CTA per SM)
   int nseg = 1;
-  {
-    const int maxseg = nk / 24 > 0 ? nk / 24 : 1;
-    double best = -1.0;
-    for (int ns = 1; ns <= maxseg; ++ns) {
-      const int ks = (nk + ns - 1) / ns, n2 = (nk + ks - 1) / ks;
-      const double waves = (double)cols * n2 / 148.0;
-      const double eff = waves / ceil(waves) * ks / (ks + 3.0);
-      if (eff > best + 1e-9) { best = eff; nseg = ns; }
-    }
+  double best = -1.0;
+  const int maxseg = nk / 24 > 0 ? nk / 24 : 1;
+  for (int ns = 1; ns <= maxseg; ++ns) {
+    const int ks = (nk + ns - 1) / ns, n2 = (nk + ks - 1) / ks;
+    const double waves = (double)cols * n2 / (148.0 * G::MINB);
+    const double eff = waves / ceil(waves) * ks / (ks + 3.0);
+    if (eff > best + 1e-9) { best = eff; nseg = ns; }
   }
   const int KS = (nk + nseg - 1) / nseg;
-  dim3 grid(ntile, (B.n[1] + 6 + VY - 1) / VY, (nk + KS - 1) / KS);
-  k_visc_march<<<grid, dim3(VX, VY), VM_SMEM, c->stream>>>(B, c->pd, B.ws, TI, KS);
+  dim3 grid(ntile, rows, (nk + KS - 1) / KS);
+  k_visc_march<G><<<grid, dim3(G::VX, G::VY), G::SMEM, c->stream>>>(B, c->pd, B.ws, TI, KS);
   c->launches++;
   return 0;
 }

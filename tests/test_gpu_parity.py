@@ -462,3 +462,38 @@ def test_profile_counts_every_hot_path_launch(po, W, B):
     g.profile_enable(False)
     g.step(1e-3)
     assert g.profile_read() == {}
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-2: on-device CFL time step (cfd_cfl_dt) against the oracle's cfl_dt (pinned by hand formula in
+# tests/test_oracle_bc_pins.py); MAX is order-independent, so the tolerance only covers sqrt / division rounding.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["c1", "multiblock", "cylinder", "ragged"])
+def test_cfl_dt_matches_oracle(po, W, B, which):
+    import torch
+
+    case = {"c1": lambda: W.c1_vortex(32), "multiblock": lambda: W.c4_multiblock(nb=12, mach=0.3),
+            "cylinder": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0, noise=1e-2),
+            "ragged": lambda: ragged_case(W, 1)}[which]()
+    o, g = pair(po, B, case)
+    for cfl in (0.5, 1.0):
+        assert abs(g.cfl_dt(cfl) / o.cfl_dt(cfl) - 1) < 1e-13
+    # after two steps (state no longer the analytic field; buffer roles exchanged by the fused stages)
+    dt = o.cfl_dt(0.5)
+    for _ in range(2):
+        o.step(dt)
+        g.step(dt)
+    assert abs(g.cfl_dt(0.5) / o.cfl_dt(0.5) - 1) < 1e-13
+    # local time step: cfl / s_i at interior points, its minimum is the global dt; ghosts untouched
+    loc = [torch.full((nk + 2 * NG, nj + 2 * NG, ni + 2 * NG), -1.0, dtype=torch.float64, device="cuda") for (ni, nj, nk) in case.dims]
+    dtg = g.cfl_dt(0.5, dt_local=loc)
+    mins = []
+    for b, a in enumerate(loc):
+        inner = a[NG:-NG, NG:-NG, NG:-NG]
+        assert (inner > 0).all()
+        mins.append(float(inner.min()))
+        a[NG:-NG, NG:-NG, NG:-NG] = -1.0
+        assert (a == -1.0).all()
+    assert abs(min(mins) / dtg - 1) < 1e-15
+    with pytest.raises(B.CfdError):
+        g.cfl_dt(0.0)
