@@ -36,7 +36,8 @@ UNIT = "Gpts/s"
 # Algorithmic flops per interior point (add, sub, mul, div, sqrt = 1 each; FMA = 2), the exact count of the
 # oracle's per-point routines run with a counting scalar (oracle/flopcount.cpp; tests/test_flopcount.py
 # checks these constants against that program).  DESIGN.md section 7.
-FLOPS_PER_POINT = {"inviscid_dir": 1381, "viscous": 478, "rk": 25, "ns_stage": 4671, "euler_stage": 4193}
+FLOPS_PER_POINT = {"inviscid_dir": 1381, "inviscid_dir_original": 1948, "viscous": 478, "rk": 25, "ns_stage": 4671,
+                   "euler_stage": 4193}
 # Algorithmic bytes per interior point per stage: read Q 5 + khat,J 10 + Q^n 5, write Q 5 doubles.
 BYTES_PER_POINT_STAGE = 200
 # FP64 ALU peak derived from unit counts and clocks: 148 SMs x 4 sub-partitions x 16 FP64
@@ -44,12 +45,18 @@ BYTES_PER_POINT_STAGE = 200
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 HBM_FALLBACK_GBS = 6650.0
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` capture (profiles/), keyed by (workload, kernel class); None until captured.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r1_marching.md: k_xi_ldg<0> at 256^3, 2.038 GB read + 1.017 GB written per launch
-    ("sweep256", "inviscid_xi"): 3.055e9,
-}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of every hot kernel, from the committed summary of the
+# `ncu --set full` capture (profiles/r2_traffic.json, written by paper_2006_07964_b200/profile_summary.py from the
+# .ncu-rep; the command is in profiles/r2_hot_kernels.md).  Keyed by workload, then kernel class; None if not captured.
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
+
+
+def load_traffic():
+    try:
+        with open(TRAFFIC_JSON) as f:
+            return json.load(f)
+    except (OSError, ValueError):
+        return {}
 
 WORKLOADS = {
     "c1": "C1 32^3 isentropic vortex, Euler, periodic, warped box",
@@ -64,23 +71,26 @@ WORKLOADS = {
 }
 
 
-def make_case(name):
+def make_case(name, scheme=0):
     from paper_2006_07964_b200 import workloads as W
 
     if name == "c1":
-        return W.c1_vortex(32)
-    if name == "c2":
-        return W.c2_freestream(64)
-    if name == "c3":
-        return W.c3_tgv(128)
-    if name == "c4":
-        return W.c4_multiblock(96)
-    if name == "c5":
-        return W.c5_cylinder()
-    if name.startswith("sweep"):
+        case = W.c1_vortex(32)
+    elif name == "c2":
+        case = W.c2_freestream(64)
+    elif name == "c3":
+        case = W.c3_tgv(128)
+    elif name == "c4":
+        case = W.c4_multiblock(96)
+    elif name == "c5":
+        case = W.c5_cylinder()
+    elif name.startswith("sweep"):
         n = int(name[5:8])
-        return W.sweep_block(n=n, viscous=0 if name.endswith("euler") else 1)
-    raise SystemExit(f"unknown workload {name}; choose from {sorted(WORKLOADS)}")
+        case = W.sweep_block(n=n, viscous=0 if name.endswith("euler") else 1)
+    else:
+        raise SystemExit(f"unknown workload {name}; choose from {sorted(WORKLOADS)}")
+    case.params["scheme"] = int(scheme)  # 0 modified AFWENO (Fig. 11), 1 original (Fig. 9)
+    return case
 
 
 def load_peaks():
@@ -146,40 +156,63 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------
 # CPU oracle arm (test infrastructure, timed as it stands: cpu_baseline and --impl reference only)
 # ---------------------------------------------------------------------------------------------------------
-def sample_case(name):
+def sample_case(name, scheme=0):
     """A BOUNDED sample of the workload for the CPU oracle: the same seeded recipe at a size that costs about
-    10-30 s of CPU work per RK3 step on one core (oracle: ~3.6 us per point-stage single-threaded)."""
+    10 s of CPU work per RK3 step on one core (oracle: ~3.6 us per point-stage single-threaded)."""
     from paper_2006_07964_b200 import workloads as W
 
     if name in ("c1", "c2"):
-        return make_case(name), f"the full workload {name}"
+        return make_case(name, scheme), f"the full workload {name}"
     if name == "c3":
-        return W.c3_tgv(96), "C3 recipe (same seed, mapping, field) generated at 96^3 instead of 128^3"
-    if name == "c4":
-        return W.c4_multiblock(48), "C4 recipe (same seed, permutations, field) with 8 blocks of 48^3 instead of 96^3"
-    if name == "c5":
-        return W.c5_cylinder(ni=256, nj=64, nk=32), "C5 recipe (same stretching ratio, BCs, noise seed) at 256x64x32"
-    n = 96
-    return (W.sweep_block(n=n, viscous=0 if name.endswith("euler") else 1),
-            f"sweep recipe (C3 seed, mapping, field) generated at {n}^3")
+        case, what = W.c3_tgv(96), "C3 recipe (same seed, mapping, field) generated at 96^3 instead of 128^3"
+    elif name == "c4":
+        case, what = W.c4_multiblock(48), "C4 recipe (same seed, permutations, field) with 8 blocks of 48^3 instead of 96^3"
+    elif name == "c5":
+        case, what = W.c5_cylinder(ni=256, nj=64, nk=32), "C5 recipe (same stretching ratio, BCs, noise seed) at 256x64x32"
+    else:
+        n = 96
+        case, what = (W.sweep_block(n=n, viscous=0 if name.endswith("euler") else 1),
+                      f"sweep recipe (C3 seed, mapping, field) generated at {n}^3")
+    case.params["scheme"] = int(scheme)
+    return case, what
 
 
-def time_oracle(name, steps, warmup, threads=None):
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def time_oracle(name, steps, warmup, threads=None, scheme=0, case=None, what=None, stages_only=0):
+    """Times the oracle as it stands.  stages_only = n > 0: n single RK stages (RHS, Eq. 20, ghost fill, BCs) instead of
+    whole RK3 steps (for the full-grid leg, where one stage is already tens of seconds of CPU work)."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import pyoracle as po
 
-    case, what = sample_case(name)
+    if case is None:
+        case, what = sample_case(name, scheme)
     o = po.Oracle(case.dims, case.faces, case.params, threads=threads)
     o.load_case(case)
     for _ in range(warmup):
         o.step(case.dt)
     t0 = time.perf_counter()
-    for _ in range(steps):
-        o.step(case.dt)
+    if stages_only:
+        for s in range(stages_only):
+            o.stage(1 + s % 3, case.dt)
+        nst = stages_only
+    else:
+        for _ in range(steps):
+            o.step(case.dt)
+        nst = 3 * steps
     el = time.perf_counter() - t0
     pts = case.npoints
-    return dict(value=pts * 3 * steps / el / 1e9, seconds=el, cores=int(o.threads), points=pts, steps=steps,
-                sample=f"{what}; {steps} RK3 step(s) = {pts * 3 * steps} point-stages", viscous=int(case.params["viscous"]))
+    return dict(value=pts * nst / el / 1e9, seconds=el, cores=int(o.threads), points=pts, steps=steps,
+                sample=f"{what}; {nst} RK stage(s) = {pts * nst} point-stages", viscous=int(case.params["viscous"]))
 
 
 def run_reference(args):
@@ -187,14 +220,15 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    r = time_oracle(args.workload, max(1, args.steps), min(args.warmup, 1))
+    r = time_oracle(args.workload, max(1, args.steps), min(args.warmup, 1), scheme=args.scheme)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": r["seconds"] / max(1, args.steps) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.workload], "name": args.workload, "stages_per_step": 3,
-                   "viscous": r["viscous"], "sample": r["sample"]},
-        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+                   "viscous": r["viscous"], "scheme": args.scheme, "sample": r["sample"]},
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+                         "cpu_model": cpu_model()},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -204,39 +238,54 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------------
 # GPU arm
 # ---------------------------------------------------------------------------------------------------------
-def dominant_roofline(prof, case, n_steps, hbm_gbs, hbm_src, dfma_probe_tflops, workload):
-    """Roofline of the dominant kernel class: algorithmic flops per launch / average launch duration (CUDA
-    events around every launch inside the timed region, cfd_profile_*), against the FP64 ALU peak; the HBM
-    term of the same kernel is reported beside it.  DESIGN.md section 7."""
+# Algorithmic bytes per interior point of the viscous point-flux kernel as designed: reads Q 5 +
+# khat 9 + J 1, writes S 4 + Fv^eta 4 + Fv^zeta 4 doubles.
+VISC_BYTES_PER_POINT = 27 * 8
+
+
+def kernel_rooflines(prof, case, n_steps, hbm_gbs, hbm_src, dfma_probe_tflops, workload):
+    """Per-kernel-class roofline from CUDA events around every launch (cfd_profile_*, a separate profiled pass after the
+    timed region): algorithmic flops (or bytes) per launch / average launch duration against the bound that applies to
+    that kernel -- the FP64 ALU peak for the sweeps, HBM for the viscous point-flux kernel (216 B and 478 flop per point:
+    33 ps vs 13 ps) and the copy kernels.  Returns (dominant, worst, table): the class with the largest share of the
+    step, the hot class furthest below its own bound, and all classes.  DESIGN.md section 7."""
     if not prof:
-        return None
+        return None, None, {}
     total_ms = sum(ms for ms, _ in prof.values())
-    name, (ms, launches) = max(prof.items(), key=lambda kv: kv[1][0])
     pts = case.npoints
-    visc = int(case.params["viscous"])
     nblocks = len(case.dims)
     pts_per_launch = pts / nblocks
-    if name.startswith("inviscid") or name.startswith("sweep"):
-        flop_pt = FLOPS_PER_POINT["inviscid_dir"]
-    elif name.startswith("rhs_fused"):
-        flop_pt = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"] - FLOPS_PER_POINT["rk"]
-    elif name.startswith("visc"):
-        flop_pt = FLOPS_PER_POINT["viscous"]
-    else:
-        flop_pt = FLOPS_PER_POINT["rk"]
-    avg_s = ms * 1e-3 / launches
-    achieved = flop_pt * pts_per_launch / avg_s / 1e12
-    traffic = NCU_TRAFFIC_BYTES.get((workload, name))
-    return {
-        "bound": "alu", "kernel": name, "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
-        "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": traffic,
-        "peak_source": "nominal FP64 FMA peak 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md s7); live DFMA probe beside it",
-        "peak_dfma_probe_tflops": dfma_probe_tflops,
-        "flop_per_point": flop_pt, "points_per_launch": pts_per_launch, "avg_launch_ms": avg_s * 1e3,
-        "launches_timed": launches, "share_of_step": ms / total_ms if total_ms > 0 else None,
-        "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
-        "kernel_ms_per_step": {k: v[0] / n_steps for k, v in prof.items()},
-    }
+    scheme = int(case.params.get("scheme", 0))
+    inv = FLOPS_PER_POINT["inviscid_dir_original" if scheme == 1 else "inviscid_dir"]
+    traffic = load_traffic().get(workload, {}) if scheme == 0 else {}
+    table = {}
+    for name, (ms, launches) in prof.items():
+        avg_s = ms * 1e-3 / launches
+        ent = {"avg_launch_ms": avg_s * 1e3, "launches_timed": launches, "share_of_step": ms / total_ms if total_ms > 0 else None,
+               "ms_per_step": ms / n_steps, "traffic": traffic.get(name)}
+        if name.startswith("inviscid"):
+            fl = inv + (FLOPS_PER_POINT["rk"] if name == "inviscid_zeta" else 0)
+            ach = fl * pts_per_launch / avg_s / 1e12
+            ent.update(bound="alu", achieved=ach, peak=FP64_PEAK_NOMINAL_TFLOPS, unit="TFLOP/s", frac=ach / FP64_PEAK_NOMINAL_TFLOPS,
+                       flop_per_point=fl)
+        elif name == "visc_flux":
+            ach = VISC_BYTES_PER_POINT * pts_per_launch / avg_s / 1e9
+            ent.update(bound="hbm", achieved=ach, peak=hbm_gbs, unit="GB/s", frac=ach / hbm_gbs, bytes_per_point=VISC_BYTES_PER_POINT,
+                       flop_per_point=FLOPS_PER_POINT["viscous"],
+                       alu_frac=FLOPS_PER_POINT["viscous"] * pts_per_launch / avg_s / 1e12 / FP64_PEAK_NOMINAL_TFLOPS)
+        else:
+            continue  # ghost fill, BC, residual: tiny launches, latency-bound; reported in kernel_ms_per_step only
+        ent["points_per_launch"] = pts_per_launch
+        table[name] = ent
+    if not table:
+        return None, None, {}
+    common = {"peak_source": "alu: nominal FP64 FMA peak 148 SM x 64 lanes x 2 x 1.965 GHz (DESIGN.md s7), live DFMA probe beside it; "
+                             f"hbm: {hbm_src}",
+              "peak_dfma_probe_tflops": dfma_probe_tflops, "hbm_peak_gbs": hbm_gbs,
+              "kernel_ms_per_step": {k: v[0] / n_steps for k, v in prof.items()}}
+    dom = max(table, key=lambda k: table[k]["ms_per_step"])
+    worst = min(table, key=lambda k: table[k]["frac"])
+    return dict(kernel=dom, **table[dom], **common), dict(kernel=worst, **table[worst]), table
 
 
 def max_over_ranks(ms, dist=None, device="cpu"):
@@ -256,12 +305,16 @@ def job_value(points_per_rank, steps, world, ms):
     return world * points_per_rank * 3 * steps / (ms * 1e-3) / 1e9
 
 
-def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, plan=0):
+def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, plan=0, scheme=0, repeats=1, keep_case=False):
+    """Timed region = `steps` RK3 steps with per-kernel event timing OFF (the shipped default path), repeated `repeats`
+    times, each repeat bracketed by barrier + synchronize and timed with CUDA events on the context's stream; the
+    reported time is the MEDIAN repeat (max over ranks of each repeat first).  The per-kernel profile is a separate pass
+    of `steps` steps after the timed region."""
     import torch
 
     from paper_2006_07964_b200 import binding as B
 
-    case = make_case(name)
+    case = make_case(name, scheme)
     ctx = B.Context(case.dims, case.faces, case.params, device=device)
     ctx.load_case(case)
     if plan:
@@ -278,9 +331,6 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, 
     for _ in range(warmup):
         ctx.step(dt)
     barrier()
-    l0 = ctx.launch_count
-    if profile:
-        ctx.profile_enable(True)
     didx = torch.device(device).index or 0
     try:
         gpu_id = "GPU-" + str(torch.cuda.get_device_properties(didx).uuid)  # robust to CUDA_VISIBLE_DEVICES remapping
@@ -289,20 +339,28 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, 
     sampler = ClockSampler(gpu_id)
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(ctx.stream)
-    for _ in range(steps):
-        ctx.step(dt)
-    e1.record(ctx.stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
+    l0 = ctx.launch_count
+    rep_ms = []
+    for _ in range(max(1, repeats)):
+        barrier()
+        e0.record(ctx.stream)
+        for _ in range(steps):
+            ctx.step(dt)
+        e1.record(ctx.stream)
+        barrier()
+        rep_ms.append(max_over_ranks(e0.elapsed_time(e1), dist, device))
+    launches = (ctx.launch_count - l0) // max(1, repeats)
     clocks = sampler.stop()
-    prof = ctx.profile_read() if profile else {}
+    ms = float(np.median(rep_ms))
+    prof = {}
     if profile:
+        ctx.profile_enable(True)
+        for _ in range(steps):
+            ctx.step(dt)
+        prof = ctx.profile_read()
         ctx.profile_enable(False)
-    launches = ctx.launch_count - l0
-    ms = max_over_ranks(ms, dist, device)
-    out = dict(case=case, ms=ms, pts=pts, launches=launches, prof=prof, clocks=clocks, finite=None)
+    out = dict(case=case if keep_case else None, dims=case.dims, params=dict(case.params), dt=case.dt, ms=ms, rep_ms=rep_ms,
+               pts=pts, launches=launches, prof=prof, clocks=clocks, finite=None)
 
     # sanity: the state must still be finite (a blown-up run would time garbage)
     out["finite"] = bool(all(torch.isfinite(ctx.interior(b, "q")).all().item() for b in range(len(case.dims))))
@@ -329,8 +387,41 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, 
         del qh
     ctx.close()
     del ctx
+    del case
     torch.cuda.empty_cache()
     return out
+
+
+class _CaseView:
+    """What kernel_rooflines needs of a case (the arrays themselves are released after the measurement)."""
+
+    def __init__(self, m):
+        self.dims, self.params, self.npoints = m["dims"], m["params"], m["pts"]
+
+
+def cpu_baseline_leg(args, gpu_value):
+    """The oracle as it stands on the host cores of this box: a bounded sample of
+    the workload on ONE core and on all cores, plus -- for the sweep workloads -- one full RK stage on the FULL grid on
+    all cores.  `value` is the all-core rate on the sample (what --impl reference also times)."""
+    one = time_oracle(args.workload, 1, 0, threads=1, scheme=args.scheme)
+    allc = time_oracle(args.workload, 1, 0, scheme=args.scheme)
+    cpu = {"value": allc["value"], "unit": UNIT, "cores": allc["cores"], "kind": "oracle", "sample": allc["sample"],
+           "seconds": allc["seconds"], "cpu_model": cpu_model(),
+           "one_core": {"value": one["value"], "unit": UNIT, "cores": 1, "seconds": one["seconds"], "sample": one["sample"],
+                        "us_per_point_stage": 1e-3 / one["value"]},
+           "gpu_over_cpu_all_cores": gpu_value / allc["value"], "gpu_over_cpu_one_core": gpu_value / one["value"],
+           "paper_context": "the paper's whole-solver speed-ups are per ONE core of a Xeon E5-2680 v3: 640x (2080 Ti), 1500x (P100), "
+                            "~2000x (Titan V) (PAPER.md L599)"}
+    if not args.no_cpu_full:
+        try:
+            full = make_case(args.workload, args.scheme)
+            r = time_oracle(args.workload, 0, 0, scheme=args.scheme, case=full, what=f"the FULL {args.workload} grid", stages_only=1)
+            cpu["full_grid_stage"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "seconds": r["seconds"],
+                                      "sample": r["sample"]}
+            del full
+        except Exception as ex:  # memory or time: the bounded legs above stand
+            cpu["full_grid_stage"] = {"error": f"{type(ex).__name__}: {ex}"[:200]}
+    return cpu
 
 
 def run_ours(args):
@@ -355,14 +446,15 @@ def run_ours(args):
 
     hbm_gbs, hbm_src = load_peaks()
     probe = B.device_peak_probe(2048)
-    main = measure_gpu(args.workload, args.steps, args.warmup, device, dist=dist, e2e=True, profile=True, plan=args.plan)
-    case, pts = main["case"], main["pts"]
-    visc = int(case.params["viscous"])
-    n_stage = 3 * args.steps
+    main = measure_gpu(args.workload, args.steps, args.warmup, device, dist=dist, e2e=True, profile=True, plan=args.plan,
+                       scheme=args.scheme, repeats=args.repeats)
+    pts = main["pts"]
+    visc = int(main["params"]["viscous"])
     value = job_value(pts, args.steps, world, main["ms"])
     e2e = main["e2e"]
     e2e_value = job_value(pts, args.steps, world, e2e["ms"])
-    flop_stage = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"]
+    inv_extra = 3 * (FLOPS_PER_POINT["inviscid_dir_original"] - FLOPS_PER_POINT["inviscid_dir"]) if args.scheme == 1 else 0
+    flop_stage = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"] + inv_extra
     per_gpu = value / world
     t_alu = flop_stage / (FP64_PEAK_NOMINAL_TFLOPS * 1e12)
     t_hbm = BYTES_PER_POINT_STAGE / (hbm_gbs * 1e9)
@@ -375,37 +467,41 @@ def run_ours(args):
             if not w or w == args.workload:
                 continue
             try:
-                r = measure_gpu(w, max(2, min(args.steps, 3)), 3, device, dist=None, e2e=False, profile=False)
-                v = r["pts"] * 3 * max(2, min(args.steps, 3)) / (r["ms"] * 1e-3) / 1e9
-                fl = FLOPS_PER_POINT["ns_stage" if int(r["case"].params["viscous"]) else "euler_stage"]
-                also[w] = {"value": v, "unit": UNIT, "points": r["pts"], "finite": r["finite"],
+                k = max(2, min(args.steps, 3))
+                r = measure_gpu(w, k, 3, device, dist=None, e2e=False, profile=False, scheme=args.scheme, repeats=3)
+                v = r["pts"] * 3 * k / (r["ms"] * 1e-3) / 1e9
+                fl = FLOPS_PER_POINT["ns_stage" if int(r["params"]["viscous"]) else "euler_stage"] + inv_extra
+                also[w] = {"value": v, "unit": UNIT, "points": r["pts"], "finite": r["finite"], "ms_per_step": r["ms"] / k,
                            "roofline_frac_stage": v * 1e9 * max(fl / (FP64_PEAK_NOMINAL_TFLOPS * 1e12), t_hbm)}
             except Exception as ex:  # a side measurement must never lose the main line
                 also[w] = {"error": f"{type(ex).__name__}: {ex}"[:200]}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        r = time_oracle(args.workload, 1, 0)
-        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
-               "seconds": r["seconds"]}
-        cpu["gpu_over_cpu"] = value / r["value"]
+        cpu = cpu_baseline_leg(args, value)
 
     if rank == 0:
+        dom, worst, table = kernel_rooflines(main["prof"], _CaseView(main), args.steps, hbm_gbs, hbm_src, probe, args.workload)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": main["ms"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.workload], "name": args.workload, "blocks": len(case.dims),
-                       "points": pts, "stages_per_step": 3, "viscous": visc, "dt": case.dt,
+            "config": {"workload": WORKLOADS[args.workload], "name": args.workload, "blocks": len(main["dims"]),
+                       "points": pts, "stages_per_step": 3, "viscous": visc, "scheme": args.scheme, "dt": main["dt"],
                        "l2_policy": "inputs larger than L2 (state+metrics per stage >> 126 MB)" if pts * 200 > 2.5e8
                        else "inputs SMALLER than L2 (small parity config; not a bandwidth claim)",
                        "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+            "timing": {"repeats": args.repeats, "statistic": "median over repeats of K steps each (max over ranks per repeat)",
+                       "ms_per_step_each_repeat": [m / args.steps for m in main["rep_ms"]],
+                       "per_kernel_profile": "separate pass after the timed region (event timing off inside it)"},
             "state_finite": main["finite"],
             "stage_roofline": {"roofline_gpts": roof_gpts, "frac": per_gpu / roof_gpts, "flop_per_point_stage": flop_stage,
                                "bytes_per_point_stage": BYTES_PER_POINT_STAGE, "alu_peak_tflops": FP64_PEAK_NOMINAL_TFLOPS,
                                "hbm_peak_gbs": hbm_gbs, "achieved_tflops": per_gpu * 1e9 * flop_stage / 1e12,
                                "achieved_alg_gbs": per_gpu * BYTES_PER_POINT_STAGE},
-            "roofline": dominant_roofline(main["prof"], case, args.steps, hbm_gbs, hbm_src, probe, args.workload),
+            "roofline": dom,
+            "roofline_worst_kernel": worst,
+            "roofline_kernels": table,
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                     "ms_per_step": e2e["ms"] / args.steps, "finite": e2e["finite"]},
@@ -426,7 +522,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="sweep256", choices=sorted(WORKLOADS))
-    ap.add_argument("--also", default="c3,c4,c5", help="comma list of extra workloads measured briefly (N=1 only)")
+    ap.add_argument("--also", default="c3,c4,c5,sweep256-euler,sweep384,sweep512",
+                    help="comma list of extra workloads measured briefly (N=1 only)")
+    ap.add_argument("--repeats", type=int, default=5, help="repeats of the timed region; the median is reported")
+    ap.add_argument("--scheme", type=int, default=0, choices=[0, 1], help="0 modified AFWENO (Fig. 11), 1 original (Fig. 9)")
+    ap.add_argument("--no-cpu-full", action="store_true", help="skip the full-grid oracle stage of the cpu_baseline leg")
     ap.add_argument("--no-also", action="store_true")
     ap.add_argument("--plan", type=int, default=0, help="cfd_set_sweep_plan (0 default; 1 all tiled; 2 all marching)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -76,7 +76,9 @@ constexpr int march_smem_doubles() {
 
 // SX (with ACC >= 1): the viscous xi term S written by k_visc_flux<true> is added to r here (the xi sweep runs first
 // and knows nothing about viscosity).
-template <int ACC, bool VISC, bool ST1, bool SX>
+// SCH: 0 = modified AFWENO (Fig. 11: eigen-system at the point, shared beta), 1 = original AFWENO (Fig. 9, NEXT-1:
+// eigen-system at the interface, two complete interpolations over j-3 .. j+2; sweep_math.cuh afweno_iface_orig).
+template <int ACC, bool VISC, bool ST1, bool SX, int SCH>
 __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
   extern __shared__ double ring[];  // thread-private columns: [RING][RV][MT] | W [2][4][MT] | out operands [2][NOUT][MT] | res [5][MT]
   using OC = OutCfg<ACC, ST1, SX>;
@@ -168,7 +170,7 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
       }
       cp_commit();
       cp_wait<1>();
-      // ---- point j: U^L_{j+1/2}, U^R_{j-1/2} ----
+      // ---- point j: U^L_{j+1/2}, U^R_{j-1/2} (SCH 0); SCH 1 forms both states of interface j-1/2 further down ----
       double Qs[5][5], UL[5], UR[5], Fc[5];
 #pragma unroll
       for (int s = 0; s < 5; ++s) {
@@ -177,7 +179,7 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
         for (int m = 0; m < 5; ++m) Qs[s][m] = sl[m * MT];
       }
       const double* sc = SLOT(j);
-      afweno_states(Qs, sc[5 * MT], sc[6 * MT], sc[7 * MT], gamma, eps4, UL, UR, Fc);
+      if (SCH == 0) afweno_states(Qs, sc[5 * MT], sc[6 * MT], sc[7 * MT], gamma, eps4, UL, UR, Fc);
       // ---- FIR: push the point flux of j+2; output = central + viscous part of Phi_{j-1/2} ----
       double G[5];
       {
@@ -198,8 +200,21 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
         const double kk = fma(kx, kx, fma(ky, ky, kz * kz));
         const double ikn = frsqrt(kk), kn = kk * ikn;
         double Fp[5], Fm[5];
-        sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
-        sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+        if (SCH == 0) {
+          sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
+          sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+        } else {
+          double Q6[6][5];
+#pragma unroll
+          for (int m = 0; m < 5; ++m) {
+            Q6[0][m] = k0[m * MT];
+#pragma unroll
+            for (int s = 0; s < 5; ++s) Q6[s + 1][m] = Qs[s][m];
+          }
+          afweno_iface_orig(Q6, kx, ky, kz, ikn, gamma, eps4, UL, UR);
+          sw_flux<+1>(UL, kx, ky, kz, kn, ikn, gamma, Fp);
+          sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+        }
         const double* so = ocol + ((j - 1) & 1) * (NOUT * MT);
         double jac = 0.0;
         if (ACC >= 2 && j > p0) jac = so[OC::O_J * MT];
@@ -226,8 +241,10 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
           Phip[m] = Phi;
         }
       }
+      if (SCH == 0) {
 #pragma unroll
-      for (int m = 0; m < 5; ++m) ULc[m] = UL[m];
+        for (int m = 0; m < 5; ++m) ULc[m] = UL[m];
+      }
     }
 #undef SLOT
   }
@@ -472,17 +489,17 @@ int pick_segments(long long ctas_per_seg, int n, int quantum) {
 
 namespace {
 
-template <int ACC, bool VISC, bool ST1, bool SX = false>
+template <int ACC, bool VISC, bool ST1, bool SX = false, int SCH = 0>
 void launch_march_k(cfd_ctx* c, const MarchArgs& A) {
   const long long lanes = (long long)A.nl * A.nt;
   dim3 grid((unsigned)((lanes + MT - 1) / MT), (unsigned)((A.n + A.S - 1) / A.S));
   const size_t smem = sizeof(double) * march_smem_doubles<ACC, VISC, ST1, SX>();
-  k_march<ACC, VISC, ST1, SX><<<grid, MT, smem, c->stream>>>(A);
+  k_march<ACC, VISC, ST1, SX, SCH><<<grid, MT, smem, c->stream>>>(A);
 }
 
-template <int ACC, bool VISC, bool ST1, bool SX = false>
+template <int ACC, bool VISC, bool ST1, bool SX = false, int SCH = 0>
 cudaError_t march_attr() {
-  return cudaFuncSetAttribute(k_march<ACC, VISC, ST1, SX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(k_march<ACC, VISC, ST1, SX, SCH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               (int)(sizeof(double) * march_smem_doubles<ACC, VISC, ST1, SX>()));
 }
 
@@ -496,6 +513,15 @@ int march_init() {
   OPT(0, false) OPT(1, false) OPT(2, false) OPT(3, false) OPT(3, true)
 #undef OPT
   if (e == cudaSuccess) e = march_attr<1, true, false, true>();
+  // scheme 1 (original AFWENO): the kernels of the default plan only
+  if (e == cudaSuccess) e = march_attr<0, false, false, false, 1>();
+  if (e == cudaSuccess) e = march_attr<1, true, false, true, 1>();
+  if (e == cudaSuccess) e = march_attr<1, false, false, false, 1>();
+#define OPT1(A, S)                                                      \
+  if (e == cudaSuccess) e = march_attr<A, true, S, false, 1>();         \
+  if (e == cudaSuccess) e = march_attr<A, false, S, false, 1>();
+  OPT1(2, false) OPT1(3, false) OPT1(3, true)
+#undef OPT1
   const int smx = (int)(sizeof(double) * XWARPS * 32 * XLS);
 #define OPTX(A)                                                                                                        \
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi<A, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx); \
@@ -508,8 +534,9 @@ int march_init() {
 // One marching sweep of block B along dir (0 xi, 1 eta, 2 zeta) with accumulation mode acc (0..2), or, with rk != null,
 // the last sweep fused with the RK stage (acc 3): the new state goes to B.r; *rk_ctas receives the number of CTAs
 // (= partial-sum groups written to rk->partials at stage 1).
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas, bool sx) {
-  const bool visc = c->pd.viscous != 0;
+// no_rows: the sweep differentiates no viscous flux rows even in a viscous run (the xi sweep of the default plan).
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas, bool sx, bool no_rows) {
+  const bool visc = c->pd.viscous != 0 && !no_rows;
   const long long o0 = B.idx(0, 0, 0);
   MarchArgs A;
   A.q = B.q + o0;
@@ -542,12 +569,25 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
     if (visc) launch_march_k<AC, true, ST>(c, A);            \
     else launch_march_k<AC, false, ST>(c, A);                \
   } while (0)
-  if (rk) { if (rk->stage == 1) GO(3, true); else GO(3, false); }
+#define GO1(AC, ST)                                          \
+  do {                                                       \
+    if (visc) launch_march_k<AC, true, ST, false, 1>(c, A);  \
+    else launch_march_k<AC, false, ST, false, 1>(c, A);      \
+  } while (0)
+  if (c->prm.scheme == 1) {  // original AFWENO (NEXT-1): default plan only (launch_rhs checks)
+    if (rk) { if (rk->stage == 1) GO1(3, true); else GO1(3, false); }
+    else if (acc == 0) launch_march_k<0, false, false, false, 1>(c, A);
+    else if (acc == 1 && sx && visc) launch_march_k<1, true, false, true, 1>(c, A);
+    else if (acc == 1) launch_march_k<1, false, false, false, 1>(c, A);
+    else GO1(2, false);
+  }
+  else if (rk) { if (rk->stage == 1) GO(3, true); else GO(3, false); }
   else if (acc == 0) GO(0, false);
   else if (acc == 1 && sx && visc) launch_march_k<1, true, false, true>(c, A);
   else if (acc == 1) GO(1, false);
   else GO(2, false);
 #undef GO
+#undef GO1
   c->launches++;
   return 0;
 }

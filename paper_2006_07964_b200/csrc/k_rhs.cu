@@ -130,7 +130,6 @@ static void visc_geometry(const BlockDev& B, bool sxi, int* T, dim3* grid, int* 
 // cfd_rhs (fused_stage 0) or, with fused_stage 1..3 (default sweep plan only), the RHS with the RK stage fused into
 // the last sweep (cfd_stage_fused): the new state lands in the r buffers and the caller exchanges the buffer roles.
 int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
-  if (c->prm.scheme != 0) { c->err = "cfd_rhs: scheme 1 (original AFWENO) is not built yet"; return CFD_E_ARG; }
   RkFuse rk;
   rk.stage = fused_stage;
   rk.dt = dt;

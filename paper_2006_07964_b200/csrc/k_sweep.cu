@@ -235,7 +235,7 @@ void launch_one(cfd_ctx* c, const BlockDev& B, bool visc) {
 }  // namespace
 
 int march_init();
-int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas, bool sx = false);
+int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* rk, int* rk_ctas, bool sx = false, bool no_rows = false);
 int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc);
 
 int sweep_init() {
@@ -257,6 +257,7 @@ int sweep_init() {
 // 3 = xi tiled and first (plain store), eta and zeta marching (zeta applies J).
 int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas) {
   if (rk && c->sweep_plan != 0) { c->err = "fused RK stage needs sweep plan 0"; return CFD_E_ARG; }
+  if (c->prm.scheme == 1 && c->sweep_plan != 0) { c->err = "scheme 1 (original AFWENO) runs on the default sweep plan only"; return CFD_E_ARG; }
   const bool visc = c->pd.viscous != 0;
   if (c->sweep_plan == 1) {
     { ProfScope ps(c, PK_INV_XI); launch_one<0, 0>(c, B, visc); }
@@ -271,8 +272,10 @@ int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas)
     {
       ProfScope ps(c, PK_INV_XI);
       const int b = (int)(&B - c->blk.data());
-      if (c->xi_mode == 1 && xi_tma_ok(c, b)) launch_xi_tma(c, b, true);
-      else if (c->xi_mode != 2 && xi_ldg_ok(c, b)) launch_xi_tma(c, b, false);
+      const bool orig = c->prm.scheme == 1;  // original AFWENO: the chunk-ring kernel or, for odd ni, the plain march
+      if (!orig && c->xi_mode == 1 && xi_tma_ok(c, b)) launch_xi_tma(c, b, true);
+      else if ((orig || c->xi_mode != 2) && xi_ldg_ok(c, b)) launch_xi_tma(c, b, false);
+      else if (orig) launch_march(c, B, 0, 0, nullptr, nullptr, false, true);
       else launch_march_xi(c, B, 0);
     }
     { ProfScope ps(c, PK_INV_ETA); launch_march(c, B, 1, 1, nullptr, nullptr, true); }

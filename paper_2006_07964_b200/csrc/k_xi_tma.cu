@@ -33,6 +33,7 @@ constexpr int PLANE = 32 * 32;              // bytes of one variable of one chun
 constexpr int SLOT = 8 * PLANE;             // Q (5) + khat (3)
 constexpr int WARP_BYTES = 3 * SLOT + 4 * PLANE;  // ring of 3 chunks + S buffer (4 rows) = 28 KB
 constexpr int XT_SMEM = TW * WARP_BYTES + 256 /*alignment slack*/ + TW * 4 * 8 /*mbarriers*/;
+constexpr int XL_SMEM = TW * 3 * SLOT + 256;  // k_xi_ldg: ring only
 
 struct XiTArgs {
   int nl, nt, n, S;     // lines (j), third extent (k), sweep length, segment length (multiple of 4)
@@ -87,7 +88,9 @@ struct XiState {
 //   PAR 1 (a odd):  P0 = (a-3, a-2), P1 = (a-1, a), P2 = (a+1, a+2)
 //   PAR 0 (a even): P0 = (a-4, a-3), P1 = (a-2, a-1), P2 = (a, a+1), P3 = (a+2, a+3)
 #define LD2(P, v) (*reinterpret_cast<const double2*>((P) + (v) * PLANE))
-template <int PAR>
+// SCH 0: modified AFWENO (eigen-system at point a, Fig. 11); SCH 1: original AFWENO (eigen-system at interface a-1/2,
+// two complete interpolations over a-3 .. a+2, Fig. 9; NEXT-1).
+template <int PAR, int SCH = 0>
 __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, const char* P2, const char* P3, bool iface, bool store,
                                         double gamma, double eps4) {
   double Qs[5][5], UL[5], UR[5], Fc[5];
@@ -102,7 +105,7 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
       Qs[0][m] = v1.x; Qs[1][m] = v1.y; Qs[2][m] = v2.x; Qs[3][m] = v2.y; Qs[4][m] = v3.x;
     }
   }
-  {
+  if (SCH == 0) {
     double kc[3];  // khat^xi at a
 #pragma unroll
     for (int c = 0; c < 3; ++c) kc[c] = PAR ? LD2(P1, 5 + c).y : LD2(P2, 5 + c).x;
@@ -130,8 +133,21 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
     const double kk = fma(kh[0], kh[0], fma(kh[1], kh[1], kh[2] * kh[2]));
     const double ikn = frsqrt(kk), kn = kk * ikn;
     double Fp[5], Fm[5];
-    sw_flux<+1>(st.ULc, kh[0], kh[1], kh[2], kn, ikn, gamma, Fp);
-    sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Fm);
+    if (SCH == 0) {
+      sw_flux<+1>(st.ULc, kh[0], kh[1], kh[2], kn, ikn, gamma, Fp);
+      sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Fm);
+    } else {
+      double Q6[6][5];
+#pragma unroll
+      for (int m = 0; m < 5; ++m) {
+        Q6[0][m] = PAR ? LD2(P0, m).x : LD2(P0, m).y;  // Q at a-3
+#pragma unroll
+        for (int t = 0; t < 5; ++t) Q6[t + 1][m] = Qs[t][m];
+      }
+      afweno_iface_orig(Q6, kh[0], kh[1], kh[2], ikn, gamma, eps4, UL, UR);
+      sw_flux<+1>(UL, kh[0], kh[1], kh[2], kn, ikn, gamma, Fp);
+      sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Fm);
+    }
     double* park = reinterpret_cast<double*>(P0) + (PAR ? 0 : 1);  // the Q words of position a-3
 #pragma unroll
     for (int m = 0; m < 5; ++m) {
@@ -140,8 +156,10 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
       st.Phip[m] = Phi;
     }
   }
+  if (SCH == 0) {
 #pragma unroll
-  for (int m = 0; m < 5; ++m) st.ULc[m] = UL[m];
+    for (int m = 0; m < 5; ++m) st.ULc[m] = UL[m];
+  }
 }
 
 // VISC: the flush adds S = d(Fv^xi)/d(xi) (rows 2..5) before the store.   r = X (+ S); the xi sweep runs first.
@@ -296,7 +314,6 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
 struct XiLArgs {
   const double* q;    // array origin (ghosts included) of the current q
   const double* kh;   // khat^xi rows
-  const double* sx;   // S rows (workspace), stored two positions to the left
   double* r;
   long long M, s1, s2;  // variable, j, k strides (doubles)
   XiTArgs g;
@@ -306,7 +323,7 @@ __device__ __forceinline__ void cp16(char* dst, const double* src) {
   asm volatile("cp.async.cg.shared.global.L2::128B [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
 
-template <bool VISC>
+template <int SCH>
 __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
   extern __shared__ char smem_raw[];
   const XiTArgs& A = L.g;
@@ -318,8 +335,7 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
   const int p0 = blockIdx.y * A.S;  // multiple of 4
   const int p1 = min(A.n, p0 + A.S);
   char* const base = smem_raw + ((256u - (smem_u32(smem_raw) & 255u)) & 255u);
-  char* const ring = base + wid * WARP_BYTES;
-  char* const sxbuf = ring + 3 * SLOT;
+  char* const ring = base + wid * (3 * SLOT);
   const int swz = (lane >> 2) & 1;
   const int off0 = lane * 32 + (swz << 4), off1 = lane * 32 + ((swz ^ 1) << 4);
   auto pair_ptr = [&](int pn) -> char* { return ring + ((pn >> 1) % 3) * SLOT + ((pn & 1) ? off1 : off0); };
@@ -348,14 +364,6 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
       for (int cc = 0; cc < 3; ++cc) cp16(slot + (5 + cc) * PLANE + soff[t], L.kh + cc * M + g);
     }
   };
-  auto load_sx = [&](int ch) {
-#pragma unroll
-    for (int t = 0; t < 2; ++t) {
-      const long long g = goff[t] + ch * 4;
-#pragma unroll
-      for (int m = 0; m < 4; ++m) cp16(sxbuf + m * PLANE + soff[t], L.sx + m * M + g);
-    }
-  };
   // r array positions 4 ch + 2 .. 4 ch + 5 are parked in the Q planes of chunk ch
   auto flush = [&](int ch, int rlo, int rhi) {  // only r positions in [rlo, rhi) are written
     const char* const slot = ring + (ch % 3) * SLOT;
@@ -367,10 +375,6 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
 #pragma unroll
       for (int m = 0; m < 5; ++m) {
         double2 v = *reinterpret_cast<const double2*>(slot + m * PLANE + soff[t]);
-        if (VISC && m > 0) {
-          const double2 sv = *reinterpret_cast<const double2*>(sxbuf + (m - 1) * PLANE + soff[t]);
-          v.x += sv.x; v.y += sv.y;
-        }
         if (rp >= rlo && rp + 1 < rhi) *reinterpret_cast<double2*>(gr + m * M) = v;
         else {
           if (rp >= rlo && rp < rhi) gr[m * M] = v.x;
@@ -422,11 +426,10 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
       if (j >= p0 + 5) flush((a >> 2) - 1, p0, p1);
       const int cn = (a >> 2) + 2;
       if (cn * 4 <= p1 + NG + 2) load_chunk(cn);
-      if (VISC) load_sx(a >> 2);
       asm volatile("cp.async.commit_group;" ::: "memory");
       last3 = j;
     }
-    xi_step<1>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4);
+    xi_step<1, SCH>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4);
     if (j + 1 <= p1) {
       const int a1 = a + 1;
       if ((a1 & 3) == 2) {  // position a1+2 opens the next chunk
@@ -434,7 +437,7 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
         __syncwarp();
       }
       P3 = pair_ptr(pb0 + ((j - (p0 - 1)) >> 1) + 3);
-      xi_step<0>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4);
+      xi_step<0, SCH>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4);
       P0 = P1; P1 = P2; P2 = P3;
     }
   }
@@ -478,8 +481,8 @@ void xi_tma_setup(cfd_ctx* c) {
   XiTmaState* S = new XiTmaState;
   S->maps.resize(c->blk.size());
   c->xi_tma = S;
-  if (cudaFuncSetAttribute(k_xi_ldg<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess ||
-      cudaFuncSetAttribute(k_xi_ldg<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess) {
+  if (cudaFuncSetAttribute(k_xi_ldg<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, XL_SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(k_xi_ldg<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, XL_SMEM) != cudaSuccess) {
     cudaGetLastError();
     return;
   }
@@ -543,10 +546,11 @@ int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
   dim3 grid((unsigned)ctas, (unsigned)((A.n + A.S - 1) / A.S));
   if (!tma) {
     XiLArgs L;
-    L.q = B.q; L.kh = B.khat; L.sx = B.ws; L.r = B.r;
+    L.q = B.q; L.kh = B.khat; L.r = B.r;
     L.M = B.M; L.s1 = B.s[1]; L.s2 = B.s[2];
     L.g = A;
-    k_xi_ldg<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(L);  // S is added by the eta sweep
+    if (c->prm.scheme == 1) k_xi_ldg<1><<<grid, 32 * TW, XL_SMEM, c->stream>>>(L);
+    else k_xi_ldg<0><<<grid, 32 * TW, XL_SMEM, c->stream>>>(L);  // the viscous xi term S is added by the eta sweep
     c->launches++;
     return 0;
   }

@@ -140,3 +140,98 @@ __device__ __forceinline__ void afweno_states(const double Qs[5][5], double kx, 
            fma(hq, a, fma(u, wx, fma(v, wy, fma(w, wz, fma(H, s, th * t)))));
   }
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// NEXT-1: the ORIGINAL AFWENO ordering (Fig. 9; reading U7) at one interface i+1/2:
+// Q6[s] = Q_{i-2+s} (s = 0..5), (kx,ky,kz) = khat_{i+1/2} (U5) with ikn = 1/|khat_{i+1/2}|.  The eigen-system is built at
+// the interface from the arithmetic mean of (rho, u, v, w, p) at i and i+1; the left state U^L_{i+1/2} comes from a
+// complete WENO interpolation on i-2..i+2, the right state U^R_{i+1/2} from another one on i-1..i+3 (nothing shared:
+// that is what the modified scheme of Fig. 11 saves).  Same algebra as afweno_states (L applied to
+// differences, R L = I for the central candidate, common-denominator weights), one side per stencil.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double weno_corr_left(double D1, double D2, double D3, double D4, double eps4) {
+  const double t1 = D2 - D1, t3 = D3 - D2, t5 = D4 - D3;
+  const double t2 = fma(3.0, D2, -D1), t4 = D2 + D3, t6 = fma(-3.0, D3, D4);
+  const double dA = fma((13.0 / 3.0) * t1, t1, fma(t2, t2, eps4));
+  const double dB = fma((13.0 / 3.0) * t3, t3, fma(t4, t4, eps4));
+  const double dC = fma((13.0 / 3.0) * t5, t5, fma(t6, t6, eps4));
+  const double pA = dB * dC, pB = dA * dC, pC = dA * dB;
+  const double sA = pA * pA, sB = (10.0 * pB) * pB, sC = pC * pC;
+  const double x = sA * (t1 - t3), y = sC * (t5 - t3);
+  return fma(0.375, x, -0.625 * y) * frcp(fma(5.0, sC, sA + sB));
+}
+__device__ __forceinline__ double weno_corr_right(double D1, double D2, double D3, double D4, double eps4) {
+  const double t1 = D2 - D1, t3 = D3 - D2, t5 = D4 - D3;
+  const double t2 = fma(3.0, D2, -D1), t4 = D2 + D3, t6 = fma(-3.0, D3, D4);
+  const double dA = fma((13.0 / 3.0) * t1, t1, fma(t2, t2, eps4));
+  const double dB = fma((13.0 / 3.0) * t3, t3, fma(t4, t4, eps4));
+  const double dC = fma((13.0 / 3.0) * t5, t5, fma(t6, t6, eps4));
+  const double pA = dB * dC, pB = dA * dC, pC = dA * dB;
+  const double sA = pA * pA, sB = (10.0 * pB) * pB, sC = pC * pC;
+  const double x = sA * (t1 - t3), y = sC * (t5 - t3);
+  return fma(0.375, y, -0.625 * x) * frcp(fma(5.0, sA, sB + sC));
+}
+
+__device__ __forceinline__ void afweno_iface_orig(const double Q6[6][5], double kx, double ky, double kz, double ikn, double gamma,
+                                                  double eps4, double UL[5], double UR[5]) {
+  const double g1 = gamma - 1.0;
+  // U7: arithmetic mean of the primitives at i (s = 2) and i+1 (s = 3)
+  double rho, u, v, w, p;
+  {
+    const double ia = frcp(Q6[2][0]), ib = frcp(Q6[3][0]);
+    const double ua = Q6[2][1] * ia, va = Q6[2][2] * ia, wa = Q6[2][3] * ia;
+    const double ub = Q6[3][1] * ib, vb = Q6[3][2] * ib, wb = Q6[3][3] * ib;
+    const double pa = g1 * fma(-0.5 * Q6[2][0], fma(ua, ua, fma(va, va, wa * wa)), Q6[2][4]);
+    const double pb = g1 * fma(-0.5 * Q6[3][0], fma(ub, ub, fma(vb, vb, wb * wb)), Q6[3][4]);
+    rho = 0.5 * (Q6[2][0] + Q6[3][0]); u = 0.5 * (ua + ub); v = 0.5 * (va + vb); w = 0.5 * (wa + wb); p = 0.5 * (pa + pb);
+  }
+  const double hq = 0.5 * fma(u, u, fma(v, v, w * w));
+  const double c2 = (gamma * p) * frcp(rho);
+  const double rsc = frsqrt(c2);
+  const double c = c2 * rsc, rc2 = rsc * rsc;
+  const double H = fma(c2, 1.0 / g1, hq);  // (e + p)/rho of the mean state
+  const double nx = kx * ikn, ny = ky * ikn, nz = kz * ikn;
+  const double th = fma(nx, u, fma(ny, v, nz * w));
+  const double b1 = g1 * rc2, hg = (0.5 * g1) * rc2, hc = 0.5 * rsc;
+  double V[5][5];  // [field][difference s: Q_{i-1+s} - Q_{i-2+s}]
+#pragma unroll
+  for (int s = 0; s < 5; ++s) {
+    const double d0 = Q6[s + 1][0] - Q6[s][0], d1 = Q6[s + 1][1] - Q6[s][1], d2 = Q6[s + 1][2] - Q6[s][2],
+                 d3 = Q6[s + 1][3] - Q6[s][3], d4 = Q6[s + 1][4] - Q6[s][4];
+    const double dx = fma(-d0, u, d1), dy = fma(-d0, v, d2), dz = fma(-d0, w, d3);
+    const double E = fma(hq, d0, d4) - fma(u, d1, fma(v, d2, w * d3));
+    const double A = fma(-b1, E, d0);
+    const double nd = fma(nx, dx, fma(ny, dy, nz * dz));
+    V[0][s] = fma(nx, A, fma(nz, dy, -ny * dz));
+    V[1][s] = fma(ny, A, fma(nx, dz, -nz * dx));
+    V[2][s] = fma(nz, A, fma(ny, dx, -nx * dy));
+    const double x = hg * E, y = hc * nd;
+    V[3][s] = x + y;
+    V[4][s] = x - y;
+  }
+  double cL[5], cR[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    cL[f] = weno_corr_left(V[f][0], V[f][1], V[f][2], V[f][3], eps4);    // stencil i-2..i+2, left state at i+1/2
+    cR[f] = weno_corr_right(V[f][1], V[f][2], V[f][3], V[f][4], eps4);   // stencil i-1..i+3, right state at i+1/2
+  }
+#pragma unroll
+  for (int side = 0; side < 2; ++side) {
+    const double* cc = side == 0 ? cL : cR;
+    double* U = side == 0 ? UL : UR;
+    const int ctr = side == 0 ? 2 : 3;  // the stencil's centre point
+    const double w1 = side == 0 ? 0.125 : -0.375, w2 = side == 0 ? 0.375 : -0.125;
+    const double a = fma(nx, cc[0], fma(ny, cc[1], nz * cc[2])), s = cc[3] + cc[4], t = c * (cc[3] - cc[4]);
+    const double wx = fma(ny, cc[2], -nz * cc[1]), wy = fma(nz, cc[0], -nx * cc[2]), wz = fma(nx, cc[1], -ny * cc[0]);
+    const double r0 = a + s;
+    double lin[5];
+#pragma unroll
+    for (int m = 0; m < 5; ++m)
+      lin[m] = fma(w1, Q6[ctr][m] - Q6[ctr - 1][m], fma(w2, Q6[ctr + 1][m] - Q6[ctr][m], Q6[ctr][m]));
+    U[0] = lin[0] + r0;
+    U[1] = lin[1] + fma(u, r0, fma(nx, t, wx));
+    U[2] = lin[2] + fma(v, r0, fma(ny, t, wy));
+    U[3] = lin[3] + fma(w, r0, fma(nz, t, wz));
+    U[4] = lin[4] + fma(hq, a, fma(u, wx, fma(v, wy, fma(w, wz, fma(H, s, th * t)))));
+  }
+}

@@ -141,7 +141,51 @@ def test_rhs_parity_other_sweep_plans(po, W, B, which, plan):
     assert_rhs_parity(o, g, case)
 
 
-def test_rhs_parity_strong_gradients(po, W, B):
+# NEXT-1: the original AFWENO ordering (scheme = 1, Fig. 9, reading U7) on the CUDA path against the oracle's
+# scheme 1 (pinned by tests/test_oracle_order.py: fifth order on a smooth line, exactness, free stream)
+@pytest.mark.parametrize("which", ["c1-euler", "tgv-ns", "ragged-ns", "ragged-euler", "ragged-even-ns", "ragged-even-euler",
+                                   "multiblock-ns", "cylinder-ns", "tiny", "strong-gradients"])
+def test_rhs_parity_scheme1_original_afweno(po, W, B, which):
+    case = {"c1-euler": lambda: W.c1_vortex(32),
+            "ragged-even-ns": lambda: ragged_case(W, 1, n=(70, 45, 9)),
+            "ragged-even-euler": lambda: ragged_case(W, 0, n=(70, 45, 9)),
+            "tgv-ns": lambda: W.tgv_sine_box(24, viscous=1, mach=0.4),
+            "ragged-ns": lambda: ragged_case(W, 1),
+            "ragged-euler": lambda: ragged_case(W, 0),
+            "multiblock-ns": lambda: W.c4_multiblock(nb=12, mach=0.3),
+            "cylinder-ns": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0, noise=1e-2),
+            "tiny": lambda: W.tgv_sine_box(6, viscous=1, mach=0.3),
+            "strong-gradients": lambda: noisy_vortex_case(W)}[which]()
+    case.params["scheme"] = 1
+    o, g = pair(po, B, case)
+    assert_rhs_parity(o, g, case)
+    # the two schemes are different discretisations: the comparison above is not vacuous
+    if which == "strong-gradients":
+        case.params["scheme"] = 0
+        o0 = po.Oracle(case.dims, case.faces, case.params)
+        o0.load_case(case)
+        o0.rhs()
+        assert np.abs(o0.interior(0, "r") - o.interior(0, "r")).max() > 1e-6 * np.abs(o.interior(0, "r")).max()
+
+
+def test_scheme1_fused_steps_match_oracle(po, W, B):
+    """Three RK3 steps with cfd_stage_fused under scheme 1 (ragged viscous block, several tiles and segments)."""
+    case = ragged_case(W, 1, n=(70, 45, 9))
+    case.params["scheme"] = 1
+    o, g = pair(po, B, case)
+    dt = o.cfl_dt(0.5)
+    for _ in range(3):
+        ro = o.step(dt)
+        rg = g.step(dt, want_res=True)
+    assert np.allclose(rg, ro, rtol=1e-10)
+    qo, qg = o.interior(0, "q"), g.to_numpy(0, "q")
+    assert np.abs(qg - qo).max() < 1e-12 * np.abs(qo).max()
+    g.set_sweep_plan(1)
+    with pytest.raises(B.CfdError):  # the tiled plans do not implement scheme 1
+        g.rhs()
+
+
+def noisy_vortex_case(W):
     """Non-smooth data (the WENO weights far from the linear ones): seeded random +-20 % perturbation per node."""
     case = W.c1_vortex(24)
     rng = np.random.default_rng(99)
@@ -149,8 +193,12 @@ def test_rhs_parity_strong_gradients(po, W, B):
     rho = q[0] * (1 + 0.2 * rng.uniform(-1, 1, q[0].shape))
     p = (1 / 1.4) * (1 + 0.2 * rng.uniform(-1, 1, q[0].shape))
     case.q0[0] = W.prim_to_cons(rho, q[1] / q[0], q[2] / q[0] + 0.3 * rng.uniform(-1, 1, q[0].shape), q[3] / q[0], p)
-    o, g = pair(po, B, case)
-    assert_rhs_parity(o, g, case)
+    return case
+
+
+def test_rhs_parity_strong_gradients(po, W, B):
+    o, g = pair(po, B, noisy_vortex_case(W))
+    assert_rhs_parity(o, g, noisy_vortex_case(W))
 
 
 def test_free_stream_on_gpu(po, W, B):
@@ -316,12 +364,14 @@ def sample_boxes(n, rng, ext=(14, 10, 8), count=5):
     return boxes, ext
 
 
-@pytest.mark.parametrize("which", ["C2-64", "C3-128", "C4-8x96", "C5-cylinder", "sweep-256"])
+@pytest.mark.parametrize("which", ["C2-64", "C3-128", "C4-8x96", "C5-cylinder", "sweep-256", "C3-128-scheme1", "sweep-256-scheme1"])
 def test_full_size_sampled_parity(po, W, B, which):
     import torch
 
     case = {"C2-64": lambda: W.c2_freestream(64), "C3-128": lambda: W.c3_tgv(128), "C4-8x96": lambda: W.c4_multiblock(96),
-            "C5-cylinder": lambda: W.c5_cylinder(), "sweep-256": lambda: W.sweep_block(256)}[which]()
+            "C5-cylinder": lambda: W.c5_cylinder(), "sweep-256": lambda: W.sweep_block(256)}[which.replace("-scheme1", "")]()
+    if which.endswith("scheme1"):
+        case.params["scheme"] = 1
     g = B.Context(case.dims, case.faces, case.params)
     g.load_case(case)
     g.step(case.dt)  # one full step first so that the sampled state is not the analytic initial field
