@@ -61,9 +61,11 @@ typedef struct {
   double reynolds; /* Re_inf */
   double prandtl;  /* Pr */
   double weno_eps; /* epsilon of Eq. 15 (1e-6) */
-  int viscous;     /* 0 Euler, 1 Navier–Stokes with constant mu = 1 (U11) */
-  int scheme;      /* 0 modified AFWENO (Fig. 11); 1 original (Fig. 9) */
+  int viscous;     /* 0 Euler, 1 Navier–Stokes */
+  int scheme;      /* 0 modified AFWENO (Fig. 11); 1 original (Fig. 9; default sweep plan only) */
   double q_inf[5]; /* far-field conservative state (rho, rho u, rho v, rho w, e) */
+  double sutherland; /* molecular viscosity (U11): > 0: Sutherland's law mu(T) = T^(3/2) (1+S)/(T+S) with
+                        S = this value = 110.4 K / T_inf (T_inf = 1, mu(1) = 1); <= 0: constant mu = 1 */
 } cfd_params;
 
 typedef struct {

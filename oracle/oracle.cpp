@@ -271,8 +271,7 @@ int Solver::rhs() {
     }
     // ---- viscous ---------------------------------------------------------------------
     if (prm.viscous) {
-      const double mu = prm.mach / prm.reynolds;                       // (Ma/Re) * mu, mu = 1 (U9, U11)
-      const double kappa = mu / (prm.prandtl * (gamma - 1.0));
+      const double mu0 = prm.mach / prm.reynolds;                      // Ma/Re: the factor of tau and q (U9)
       // pass A (cuda_vars_derv_xyz, Fig. 12): Cartesian gradients of (u,v,w,T) on interior + 3 face layers
       std::vector<double> G(12 * M, 0.0);
 #pragma omp parallel for schedule(static) num_threads(nthreads)
@@ -318,6 +317,8 @@ int Solver::rhs() {
                 kd[c] = B.khat[(d * 3 + c) * M + p];
                 for (int f = 0; f < 4; ++f) g[c][f] = G[(c * 4 + f) * M + p];
               }
+              const double mu = mu0 * sutherland_mu(ph[3], prm.sutherland);   // (Ma/Re) mu(T); mu = 1 without Sutherland (U11)
+              const double kappa = mu / (prm.prandtl * (gamma - 1.0));
               visc_flux_point(ph, g, kd, mu, kappa, F);
               for (int m = 0; m < 5; ++m) Fv[m * M + p] = F[m];
             }
@@ -551,6 +552,7 @@ void orc_visc_flux_point(const double* vel, const double* g, const double* k, do
   std::memcpy(gg, g, sizeof(gg));
   visc_flux_point(vel, gg, k, mu, kappa, Fv);
 }
+double orc_sutherland_mu(double T, double S) { return sutherland_mu(T, S); }
 void orc_grad_point(const double* dphi, const double* kh, double J, double* g) {
   double a[3][4], b[3][3], o[3][4];
   std::memcpy(a, dphi, sizeof(a));

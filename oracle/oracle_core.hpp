@@ -44,9 +44,10 @@ enum FaceType { FT_NONE = 0, FT_PERIODIC = 1, FT_INTERFACE = 2, FT_WALL = 3, FT_
 
 struct Params {
   double gamma, mach, reynolds, prandtl, weno_eps;
-  int viscous;  // 0 Euler, 1 Navier–Stokes with constant mu = 1 (U11)
+  int viscous;  // 0 Euler, 1 Navier–Stokes
   int scheme;   // 0 modified AFWENO (Fig. 11), 1 original (Fig. 9)
   double q_inf[5];
+  double sutherland;  // S / T_inf of Sutherland's law (U11); <= 0: constant mu = 1
 };
 
 struct Face {
@@ -350,6 +351,14 @@ inline void grad_point(const T dphi[3][4], const T kh[3][3], const T& J, T g[3][
   for (int c = 0; c < 3; ++c)
     for (int f = 0; f < 4; ++f)
       g[c][f] = J * ((kh[0][c] * dphi[0][f] + kh[1][c] * dphi[1][f]) + kh[2][c] * dphi[2][f]);
+}
+
+// Molecular viscosity mu(T) ("molecular viscosity mu" stored per point; reading U11, NEXT-3): Sutherland's law in
+// the reference scales (T_inf = 1, mu(1) = 1):  mu = T^(3/2) (1 + S) / (T + S),  S = 110.4 K / T_inf;  S <= 0: mu = 1.
+template <class T>
+inline T sutherland_mu(const T& Tt, double S) {
+  if (!(S > 0.0)) return T(1.0);
+  return Tt * sqrt(Tt) * T(1.0 + S) / (Tt + T(S));
 }
 
 // O3 (second half): point viscous flux along direction with hatted metrics k (Eqs. 5–6,

@@ -23,7 +23,8 @@ NG = 6
 
 class _Params(C.Structure):
     _fields_ = [("gamma", C.c_double), ("mach", C.c_double), ("reynolds", C.c_double), ("prandtl", C.c_double),
-                ("weno_eps", C.c_double), ("viscous", C.c_int), ("scheme", C.c_int), ("q_inf", C.c_double * 5)]
+                ("weno_eps", C.c_double), ("viscous", C.c_int), ("scheme", C.c_int), ("q_inf", C.c_double * 5),
+                ("sutherland", C.c_double)]
 
 
 class _Face(C.Structure):
@@ -68,6 +69,8 @@ def lib():
         L.orc_inviscid_line.argtypes = [C.c_int, dp, dp, C.c_double, C.c_double, C.c_int, dp]
         L.orc_visc_flux_point.argtypes = [dp, dp, dp, C.c_double, C.c_double, dp]
         L.orc_grad_point.argtypes = [dp, dp, C.c_double, dp]
+        L.orc_sutherland_mu.argtypes = [C.c_double, C.c_double]
+        L.orc_sutherland_mu.restype = C.c_double
         _lib = L
     return _lib
 
@@ -130,6 +133,10 @@ def visc_flux_point(vel, g, k, mu, kappa):
     return Fv
 
 
+def sutherland_mu(T, S):
+    return lib().orc_sutherland_mu(float(T), float(S))
+
+
 def grad_point(dphi, kh, J):
     g = np.zeros((3, 4))
     lib().orc_grad_point(_f64(dphi), _f64(kh), J, g)
@@ -158,6 +165,7 @@ class Oracle:
             setattr(p, k, params[k])
         for a in range(5):
             p.q_inf[a] = params["q_inf"][a]
+        p.sutherland = float(params.get("sutherland", 0.0))
         self.h = L.orc_create(nb, d, len(faces), fa, C.byref(p))
         if not self.h:
             raise ValueError("orc_create failed (see stderr)")

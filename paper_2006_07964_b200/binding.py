@@ -37,7 +37,8 @@ class _Dims(C.Structure):
 
 class _Params(C.Structure):
     _fields_ = [("gamma", C.c_double), ("mach", C.c_double), ("reynolds", C.c_double), ("prandtl", C.c_double),
-                ("weno_eps", C.c_double), ("viscous", C.c_int), ("scheme", C.c_int), ("q_inf", C.c_double * 5)]
+                ("weno_eps", C.c_double), ("viscous", C.c_int), ("scheme", C.c_int), ("q_inf", C.c_double * 5),
+                ("sutherland", C.c_double)]
 
 
 class _Face(C.Structure):
@@ -141,6 +142,7 @@ class Context:
                 setattr(p, k, params[k])
             for a in range(5):
                 p.q_inf[a] = params["q_inf"][a]
+            p.sutherland = float(params.get("sutherland", 0.0))
             fa = (_Face * max(1, len(faces)))()
             for t, f in enumerate(faces):
                 fa[t].block, fa[t].face, fa[t].type = f["block"], f["face"], f["type"]

@@ -116,6 +116,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   c->pd.viscous = params->viscous;
   c->pd.mu = params->viscous ? params->mach / params->reynolds : 0.0;
   c->pd.kappa = params->viscous ? c->pd.mu / (params->prandtl * (params->gamma - 1.0)) : 0.0;
+  c->pd.suth = params->sutherland > 0.0 ? params->sutherland : 0.0;
   for (int m = 0; m < 5; ++m) c->pd.q_inf[m] = params->q_inf[m];
   c->stream = (cudaStream_t)cuda_stream;
   c->blk.resize(nblocks);

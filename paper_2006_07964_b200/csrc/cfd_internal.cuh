@@ -26,7 +26,8 @@ struct BlockDev {
 };
 
 struct ParamsDev {
-  double gamma, eps, mu, kappa;  // mu = Ma/Re (mu == 1, U9/U11), kappa = mu / (Pr (gamma-1))
+  double gamma, eps, mu, kappa;  // mu = Ma/Re (U9), kappa = mu / (Pr (gamma-1)); both times mu(T) when suth > 0
+  double suth;                   // Sutherland's S / T_inf (U11); <= 0: constant mu = 1
   double q_inf[5];
   int viscous;
 };

@@ -23,3 +23,8 @@ __device__ __forceinline__ double frsqrt(double x) {
   const double p = fma(0.375, e, 0.5);
   return fma(y, p * e, y);
 }
+
+// Sutherland's law in the reference scales (U11): mu(T)/mu(1) = T^(3/2) (1 + S) / (T + S), S > 0.
+__device__ __forceinline__ double sutherland_factor(double T, double S) {
+  return (T * (T * frsqrt(T))) * ((1.0 + S) * frcp(T + S));
+}

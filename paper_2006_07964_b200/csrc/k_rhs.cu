@@ -77,7 +77,11 @@ __global__ void __launch_bounds__(256) k_visc_flux(BlockDev B, ParamsDev P, cons
 #pragma unroll
       for (int f = 0; f < 4; ++f) g[c][f] = J * ((kh[0][c] * dphi[0][f] + kh[1][c] * dphi[1][f]) + kh[2][c] * dphi[2][f]);
     const double u = phi[p], v = phi[M + p], w = phi[2 * M + p];
-    const double mu = P.mu, kap = P.kappa;
+    double mu = P.mu, kap = P.kappa;
+    if (P.suth > 0.0) {  // mu(T) by Sutherland's law (U11)
+      const double f = sutherland_factor(phi[3 * M + p], P.suth);
+      mu *= f; kap *= f;
+    }
     const double div = g[0][0] + g[1][1] + g[2][2];
     const double lam = -(2.0 / 3.0) * mu;
     const double txx = lam * div + 2.0 * mu * g[0][0];

@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
     }
   }
   stage(kb);
-  const double mu = P.mu, kap = P.kappa, lam = -(2.0 / 3.0) * mu;
+  const double mu0 = P.mu, kap0 = P.kappa, suth = P.suth;
   auto s_of_plane = [&](int kk) {
     if (own && !oj && col_in && kk >= 0 && kk < B.n[2]) {
       const long long p = pcol + (long long)(kk + NG) * s2;
@@ -184,6 +184,12 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
         for (int c = 0; c < 3; ++c) g[c][f] = J * ((kh[0][c] * dx + kh[1][c] * dy) + kh[2][c] * dz);
       }
       const double u = ph[3][0], v = ph[3][1], w = ph[3][2];
+      double mu = mu0, kap = kap0;
+      if (suth > 0.0) {  // mu(T) by Sutherland's law (U11): uniform branch
+        const double f = sutherland_factor(ph[3][3], suth);
+        mu *= f; kap *= f;
+      }
+      const double lam = -(2.0 / 3.0) * mu;
       const double div = g[0][0] + g[1][1] + g[2][2];
       const double txx = lam * div + 2.0 * mu * g[0][0];
       const double tyy = lam * div + 2.0 * mu * g[1][1];

@@ -40,11 +40,12 @@ class Case:
         return int(sum(a * b * c for a, b, c in self.dims))
 
 
-def default_params(viscous=0, mach=0.5, reynolds=1600.0, prandtl=0.71, q_inf=None, scheme=0):
+def default_params(viscous=0, mach=0.5, reynolds=1600.0, prandtl=0.71, q_inf=None, scheme=0, sutherland=0.0):
     if q_inf is None:
         q_inf = prim_to_cons(1.0, mach, 0.0, 0.0, 1.0 / GAMMA)
     return dict(gamma=GAMMA, mach=float(mach), reynolds=float(reynolds), prandtl=float(prandtl),
-                weno_eps=1e-6, viscous=int(viscous), scheme=int(scheme), q_inf=[float(x) for x in q_inf])
+                weno_eps=1e-6, viscous=int(viscous), scheme=int(scheme), q_inf=[float(x) for x in q_inf],
+                sutherland=float(sutherland))
 
 
 def prim_to_cons(rho, u, v, w, p):
@@ -355,3 +356,36 @@ def tgv_sine_box(n=16, viscous=1, mach=0.1, amp=0.1):
     return Case("tgv-sine-box", [(n, n, n)], [xyz], [q0], periodic_faces(0, (L, L, L)),
                 default_params(viscous=viscous, mach=mach, reynolds=1600.0, prandtl=0.71),
                 dt=0.5 * 0.75 * h / (1.0 + mach) / 1.8, steps=0, meta=dict(L=L, h=h))
+
+
+def shock_vortex(n=48, viscous=1, sutherland=110.4 / 288.15, seed=SEED0 + 6, pressure_ratio=6.0, density_ratio=4.0,
+                 strength=1.5, reynolds=500.0, steps=50):
+    """Shocked periodic workload (the paper's target flows are supersonic jets): a
+    high-pressure slab x in [L/4, 3L/4) of the seeded wavy periodic box (two shock / contact / rarefaction systems, the
+    initial jumps are steps that cut the curvilinear grid lines obliquely) with an isentropic vortex (axis || z, radius
+    scale 0.5) inside the slab and a weak spanwise velocity, so that the nonlinear WENO weights work far from the smooth
+    limit in all three sweeps (shock Mach number ~ 1.35 for the default jumps; ratios of 10 / 8 blow up with this
+    scheme's unlimited central terms).  Navier–Stokes with Sutherland viscosity (or Euler with viscous=0)."""
+    L = 2 * np.pi
+    xyz, h, _ = wavy_box(n, seed, L)
+    x, y, z = xyz
+    g = GAMMA
+    inside = (x % L >= 0.25 * L) & (x % L < 0.75 * L)
+    rho_b = np.where(inside, 1.0, 1.0 / density_ratio)
+    p_b = np.where(inside, 1.0 / g, 1.0 / (g * pressure_ratio))
+    T_b = g * p_b / rho_b
+    r0 = 0.5
+    xb = (x - 0.5 * L) / r0
+    yb = ((y - 0.5 * L + 0.5 * L) % L - 0.5 * L) / r0
+    r2 = xb * xb + yb * yb
+    f = strength / (2 * np.pi) * np.exp(0.5 * (1.0 - r2))
+    u = -f * yb
+    v = f * xb
+    w = 0.05 * np.sin(z) * np.cos(y)
+    T = T_b * (1.0 - (g - 1.0) * strength ** 2 / (8 * np.pi ** 2) * np.exp(1.0 - r2))
+    rho = rho_b * (T / T_b) ** (1.0 / (g - 1.0))
+    p = rho * T / g
+    q0 = prim_to_cons(rho, u, v, w, p)
+    prm = default_params(viscous=viscous, mach=1.0, reynolds=reynolds, prandtl=0.71, sutherland=sutherland if viscous else 0.0)
+    return Case("shock-vortex", [tuple([n] * 3)], [xyz], [q0], periodic_faces(0, (L, L, L)), prm,
+                dt=0.4 * 0.75 * h / 2.2 / 1.8, steps=steps, meta=dict(L=L, h=h))

@@ -1,0 +1,196 @@
+"""GPU parity at CONFIG SIZE and CONFIG LENGTH (-m gpu; several minutes of oracle time on the host cores): the runs
+BASELINE.json's configs name, advanced for many steps in the launch configuration bench.py times, against the CPU
+oracle (north_star: "1e-10 after 100 RK steps on smooth cases", "on all five workloads").
+
+  C3  128^3 Taylor-Green, 100 RK3 steps: state vs oracle at 1e-10 max|Q|; kinetic energy and enstrophy every 10 steps vs
+      the oracle's, and the t = 0 closed forms <|u|^2>/2 = Ma^2/8, <|omega|^2>/2 = 3 Ma^2/8.
+  C4  8 x 96^3 with signed permutations, 20 RK3 steps: state vs oracle; and the 8-block GPU run equals the single-block
+      192^3 GPU run of the same global field (pin 7 on the CUDA path).
+  C5  cylinder 1024 x 256 x 128 after the 50 steps of the config: state finite, RHS parity on sampled sub-boxes (wall,
+      far field, interior), boundary ghosts consistent.
+  S1  full-size metrics: the oracle recomputes khat, J from the GPU's own xyz sub-box (ghosts included) for C4 and C5.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+NG = 6
+GAMMA = 1.4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2006_07964_b200 import binding
+
+    return binding
+
+
+def _d6(a, axis):
+    """6th-order central difference with periodic wrap (test-side analysis of a periodic interior array)."""
+    r = lambda s: np.roll(a, -s, axis=axis)
+    return 0.75 * (r(1) - r(-1)) - 0.15 * (r(2) - r(-2)) + (1.0 / 60.0) * (r(3) - r(-3))
+
+
+def tgv_diagnostics(q, khat, jac):
+    """Volume averages on a periodic curvilinear block: (<|u|^2>/2, <rho |u|^2>/2, <|omega|^2>/2) with dV = 1/J,
+    du_a/dx_c = J sum_d khat^d_c delta_d u_a (Eq. 21).  q [5,k,j,i], khat [9,k,j,i], jac [k,j,i] (interior)."""
+    rho = q[0]
+    u = q[1:4] / rho
+    kh = khat.reshape(3, 3, *rho.shape)
+    du = np.zeros((3, 3) + rho.shape)  # [a][c] = du_a/dx_c
+    for a in range(3):
+        dd = [_d6(u[a], axis=2), _d6(u[a], axis=1), _d6(u[a], axis=0)]  # xi = last array axis
+        for c in range(3):
+            du[a, c] = jac * (kh[0, c] * dd[0] + kh[1, c] * dd[1] + kh[2, c] * dd[2])
+    om = np.stack([du[2, 1] - du[1, 2], du[0, 2] - du[2, 0], du[1, 0] - du[0, 1]])
+    w = 1.0 / jac
+    vol = w.sum()
+    u2 = (u ** 2).sum(0)
+    return np.array([(0.5 * u2 * w).sum() / vol, (0.5 * rho * u2 * w).sum() / vol, (0.5 * (om ** 2).sum(0) * w).sum() / vol])
+
+
+def test_c3_128_hundred_steps_state_and_tgv_diagnostics(po, W, B):
+    case = W.c3_tgv(128)
+    ma = case.params["mach"]
+    o = po.Oracle(case.dims, case.faces, case.params)
+    o.load_case(case)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    kh, J = o.interior(0, "khat"), o.interior(0, "jac")[0]
+    d0 = tgv_diagnostics(o.interior(0, "q"), kh, J)
+    assert abs(d0[0] / (ma ** 2 / 8) - 1) < 1e-6          # <|u|^2>/2 = Ma^2/8 exactly for the TGV field
+    assert abs(d0[1] / (ma ** 2 / 8) - 1) < 2 * ma ** 2    # E_k = Ma^2/8 (1 + O(Ma^2))
+    assert abs(d0[2] / (3 * ma ** 2 / 8) - 1) < 1e-6       # enstrophy = 3 Ma^2/8
+    dt = g.cfl_dt(0.5)
+    assert abs(dt / o.cfl_dt(0.5) - 1) < 1e-13
+    for step in range(1, 101):
+        o.step(dt)
+        g.step(dt)
+        if step % 10 == 0:
+            qo, qg = o.interior(0, "q"), g.to_numpy(0, "q")
+            do, dg = tgv_diagnostics(qo, kh, J), tgv_diagnostics(qg, kh, J)
+            assert np.abs(dg / do - 1).max() < 1e-10, (step, do, dg)
+            assert np.abs(qg - qo).max() < 1e-10 * np.abs(qo).max(), step
+    # the flow has started to evolve (not a frozen field): kinetic energy decays, enstrophy grows (Re = 1600)
+    assert do[1] < d0[1] and do[2] > d0[2]
+
+
+def test_c4_8x96_twenty_steps_vs_oracle_and_vs_single_block_192(po, W, B):
+    import torch
+
+    case = W.c4_multiblock(96)
+    o = po.Oracle(case.dims, case.faces, case.params)
+    o.load_case(case)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    L, G = case.meta["L"], case.meta["G"]
+    single = W.Case("C4-single-192", [tuple(G)], [case.meta["xyz_g"]], [case.meta["q_g"]], W.periodic_faces(0, (L, L, L)),
+                    dict(case.params), dt=case.dt, steps=0)
+    g1 = B.Context(single.dims, single.faces, single.params)
+    g1.load_case(single)
+    dt = g.cfl_dt(0.5)
+    assert abs(dt / o.cfl_dt(0.5) - 1) < 1e-13
+    assert abs(g1.cfl_dt(0.5) / dt - 1) < 1e-12   # same global field: same time step up to the metrics' round-off
+    for _ in range(20):
+        ro = o.step(dt)
+        rg = g.step(dt, want_res=True)
+        r1 = g1.step(dt, want_res=True)
+    assert np.allclose(rg, ro, rtol=1e-9)
+    assert np.allclose(rg, r1, rtol=1e-9)
+    scale = max(np.abs(o.interior(b, "q")).max() for b in range(8))
+    for b in range(8):
+        assert np.abs(g.to_numpy(b, "q") - o.interior(b, "q")).max() < 1e-11 * scale, b
+    glob = W.gather_blocks([g.to_numpy(b, "q") for b in range(8)], case.meta["info"], G)
+    one = g1.to_numpy(0, "q")
+    assert np.abs(glob - one).max() < 1e-11 * scale
+    torch.cuda.synchronize()
+
+
+def _subbox_rhs_and_metrics(po, g, case, b, lo, ext, S, check_metrics):
+    sl = tuple(slice(lo[a], lo[a] + ext[a] + 2 * NG) for a in (2, 1, 0))
+    o = po.Oracle([tuple(ext)], [], case.params)
+    if check_metrics:
+        # S1 at full size: the oracle differentiates the GPU's own coordinates (ghost layers included)
+        o.field(0, "xyz")[...] = g.field(b, "xyz")[(slice(None),) + sl].cpu().numpy()
+        o.compute_metrics()
+        box = (slice(None),) + (slice(3, -3),) * 3
+        ko = o.field(0, "khat")[box]
+        kg = g.field(b, "khat")[(slice(None),) + sl].cpu().numpy()[box]
+        assert np.abs(kg - ko).max() < 1e-13 * np.abs(ko).max(), (case.name, b, lo)
+        jo = o.field(0, "jac")[box]
+        jg = g.field(b, "jac")[(slice(None),) + sl].cpu().numpy()[box]
+        assert np.abs(jg / jo - 1).max() < 1e-12, (case.name, b, lo)
+    else:
+        for name in ("khat", "jac"):
+            o.field(0, name)[...] = g.field(b, name)[(slice(None),) + sl].cpu().numpy()
+    o.field(0, "q")[...] = g.field(b, "q")[(slice(None),) + sl].cpu().numpy()
+    o.rhs()
+    isl = tuple(slice(lo[a] + NG, lo[a] + NG + ext[a]) for a in (2, 1, 0))
+    rg = g.field(b, "r")[(slice(None),) + isl].cpu().numpy()
+    err = np.abs(rg - o.interior(0, "r")).max(axis=(1, 2, 3)) / S
+    assert err.max() < 1e-12, (case.name, b, lo, err)
+
+
+def _flux_scale(g, b):
+    q = g.interior(b, "q")
+    u = q[1:4] / q[0]
+    p = (GAMMA - 1) * (q[4] - 0.5 * q[0] * (u ** 2).sum(0))
+    kh = g.interior(b, "khat").reshape(3, 3, *q.shape[1:])
+    J = g.interior(b, "jac")[0]
+    S = np.zeros(5)
+    for d in range(3):
+        th = (kh[d] * u).sum(0)
+        F = [q[0] * th, q[1] * th + kh[d, 0] * p, q[2] * th + kh[d, 1] * p, q[3] * th + kh[d, 2] * p, (q[4] + p) * th]
+        S = np.maximum(S, np.array([float(f.abs().max()) for f in F]))
+    return S * float(J.max())
+
+
+def test_c5_cylinder_after_the_fifty_steps_of_the_config(po, W, B):
+    import torch
+
+    case = W.c5_cylinder()
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    for _ in range(case.steps):  # 50 RK3 steps
+        g.step(case.dt)
+    g.rhs()
+    torch.cuda.synchronize()
+    q = g.interior(0, "q")
+    assert torch.isfinite(q).all()
+    assert float(q[0].min()) > 0.5 and float(q[0].max()) < 2.0
+    # wall nodes stay at rest; the flow near the wall has developed (no longer the impulsive start)
+    assert float(q[1:4, :, 0, :].abs().max()) == 0.0
+    assert float((q[1, :, 1, :] / q[0, :, 1, :]).abs().max()) < case.params["mach"]
+    S = _flux_scale(g, 0)
+    n = case.dims[0]
+    ext = (14, 10, 8)
+    rng = np.random.default_rng(77)
+    boxes = [(0, 0, 0), (n[0] - ext[0], n[1] - ext[1], n[2] - ext[2]),           # wall corner, far-field corner
+             (500, 0, 60), (100, n[1] - ext[1], 3)]                              # mid wall, mid far field
+    boxes += [tuple(int(rng.integers(0, n[a] - ext[a] + 1)) for a in range(3)) for _ in range(4)]
+    for lo in boxes:
+        _subbox_rhs_and_metrics(po, g, case, 0, lo, ext, S, check_metrics=True)
+
+
+def test_c4_full_size_metrics_from_gpu_coordinates(po, W, B):
+    import torch
+
+    case = W.c4_multiblock(96)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    g.step(case.dt)
+    g.rhs()
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(78)
+    ext = (14, 10, 8)
+    for b in (0, 3, 5, 7):
+        S = _flux_scale(g, b)
+        n = case.dims[b]
+        boxes = [(0, 0, 0), tuple(n[a] - ext[a] for a in range(3))]
+        boxes += [tuple(int(rng.integers(0, n[a] - ext[a] + 1)) for a in range(3)) for _ in range(2)]
+        for lo in boxes:
+            _subbox_rhs_and_metrics(po, g, case, b, lo, ext, S, check_metrics=True)

@@ -98,6 +98,9 @@ def _analytic_viscous_rhs(xyz, params):
     p = sp.Rational(5, 7) * (1 + sp.Rational(1, 20) * sp.sin(2 * x) * sp.cos(y) * sp.sin(z))
     T = g * p / rho
     mu = sp.Float(Ma) / sp.Float(Re)
+    S = float(params.get("sutherland", 0.0))
+    if S > 0:  # Sutherland's law in the reference scales (U11): mu(T) = T^(3/2) (1 + S) / (T + S)
+        mu = mu * T ** sp.Rational(3, 2) * (1 + sp.Float(S)) / (T + sp.Float(S))
     vel, X = [u, v, w], [x, y, z]
     div = sum(sp.diff(vel[i], X[i]) for i in range(3))
     tau = [[mu * (sp.diff(vel[i], X[j]) + sp.diff(vel[j], X[i]) - (sp.Rational(2, 3) * div if i == j else 0)) for j in range(3)]
@@ -110,13 +113,16 @@ def _analytic_viscous_rhs(xyz, params):
     return np.stack(out[:4]), out[4:]
 
 
-def test_viscous_operator_converges_to_analytic_navier_stokes(po, W):
-    """R_NS - R_Euler (the oracle's S3) vs the analytic viscous terms on a warped periodic grid: order -> 6."""
+@pytest.mark.parametrize("sutherland", [0.0, 0.4])
+def test_viscous_operator_converges_to_analytic_navier_stokes(po, W, sutherland):
+    """R_NS - R_Euler (the oracle's S3) vs the analytic viscous terms on a warped periodic grid: order -> 6.
+    sutherland = 0.4 (= 110.4 K / 276 K): the same with mu(T) by Sutherland's law inside the analytic stresses and heat
+    flux (T varies by +-15 % in this field, so mu varies by ~ +-11 %: a missing or misplaced mu(T) is an O(10 %) error)."""
     errs = []
     Ns = (12, 18, 27)
     for n in Ns:
         base = W.tgv_sine_box(n, viscous=1, amp=0.15)
-        base.params.update(mach=1.0, reynolds=100.0)  # mu_eff = 0.01
+        base.params.update(mach=1.0, reynolds=100.0, sutherland=sutherland)  # mu_eff = 0.01 mu(T)
         ref, (rho, u, v, w, p) = _analytic_viscous_rhs(base.xyz[0], base.params)
         base.q0[0] = W.prim_to_cons(rho, u, v, w, p)
         r = {}

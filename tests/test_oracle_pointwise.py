@@ -308,3 +308,22 @@ def test_visc_flux_pure_shear_and_dilatation(po):
     g[:, :3] = rng.normal(size=(3, 3))
     tr = sum(po.visc_flux_point([0, 0, 0], g, np.eye(3)[c], mu, kappa)[1 + c] for c in range(3))
     assert abs(tr) < 1e-16
+
+
+def test_sutherland_law_closed_forms(po):
+    """mu(T) = T^(3/2) (1 + S)/(T + S) in the reference scales (U11): mu(1) = 1 for every S, hand values,
+    the classical dimensional ratio for air, and S <= 0 switches it off (constant mu = 1)."""
+    for S in (0.1, 0.4, 110.4 / 288.15, 2.0):
+        assert abs(po.sutherland_mu(1.0, S) - 1.0) < 1e-15
+    assert abs(po.sutherland_mu(2.0, 0.4) - 2.0 ** 1.5 * 1.4 / 2.4) < 1e-15
+    assert abs(po.sutherland_mu(0.25, 0.5) - 0.125 * 1.5 / 0.75) < 1e-15
+    # air, T_inf = 273.15 K, S = 110.4 K: mu(373.15 K)/mu(273.15 K) = (373.15/273.15)^1.5 (273.15 + 110.4)/(373.15 + 110.4)
+    S = 110.4 / 273.15
+    want = (373.15 / 273.15) ** 1.5 * (273.15 + 110.4) / (373.15 + 110.4)
+    assert abs(po.sutherland_mu(373.15 / 273.15, S) / want - 1) < 1e-14
+    for T in (0.3, 1.0, 4.0):
+        assert po.sutherland_mu(T, 0.0) == 1.0 and po.sutherland_mu(T, -1.0) == 1.0
+    # monotone in T
+    Ts = np.linspace(0.2, 5.0, 50)
+    mus = np.array([po.sutherland_mu(t, 0.4) for t in Ts])
+    assert (np.diff(mus) > 0).all()
