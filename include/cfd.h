@@ -17,9 +17,13 @@
  *  - Layout of every field: fp64, structure-of-arrays [var][k][j][i], i fastest, each axis
  *    carrying CFD_NG = 6 ghost layers on both sides: extents (ni+12, nj+12, nk+12),
  *    M = (ni+12)(nj+12)(nk+12) doubles per variable.  Pointers must be 16-byte aligned.
- *  - All work is enqueued on the CUDA stream given to cfd_create_blocks; no function
- *    synchronises the device unless documented ("returns host values").
- *  - No cudaMalloc/cudaFree after cfd_create_blocks (which allocates a few KB of descriptors).
+ *  - All work is ordered on the CUDA stream given to cfd_create_blocks: it is enqueued there or, for contexts
+ *    with more than one block, partly on four library-owned non-blocking side streams that cfd_rhs /
+ *    cfd_stage_fused fork from that stream and join back into it before they return (the blocks' kernel chains
+ *    run concurrently; work enqueued on the caller's stream before or after a call is ordered with it).  No
+ *    function synchronises the device unless documented ("returns host values").
+ *  - No cudaMalloc/cudaFree after cfd_create_blocks (which allocates a few KB of descriptors and, for
+ *    multi-block contexts, the side streams and their events).
  *  - There is no CPU fallback: without a CUDA device cfd_create_blocks fails with CFD_E_CUDA.
  * ===================================================================================== */
 #ifndef CFD_B200_H
@@ -87,15 +91,17 @@ typedef struct {
   double* jac;  /* [1][M] J (Eq. 8) */
 } cfd_block_ptrs;
 
-/* Bytes of device scratch the caller must pass to cfd_create_blocks: 16 doubles per stored point of EVERY block
+/* Bytes of device scratch the caller must pass to cfd_create_blocks: 12 doubles per stored point of EVERY block
  * (each block has its own area, so that the per-block kernels of a multi-block case can run concurrently: the
- * viscous rows S, Fv^eta, Fv^zeta; phi = (u,v,w,T) for the tiled plans; the 9 metric first derivatives during
- * cfd_compute_metrics), plus the partial sums of the residual reduction. */
+ * viscous rows S = d(Fv^xi)/d(xi), Fv^eta, Fv^zeta; the 9 metric first derivatives during cfd_compute_metrics),
+ * plus the partial sums of the residual / CFL reductions. */
 size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params* params);
 
 /* Build a context over nblocks point-matched blocks (a patch is a whole block face).
- * Validates sizes, alignment and the face descriptors (permutation proper, normal-axis sign
- * consistent with the face pair, tangential extents equal).  `workspace` is device memory of at
+ * Validates sizes, alignment and the face descriptors: all six faces of every block described exactly once,
+ * permutation proper, normal-axis sign consistent with the face pair, tangential extents equal, the two sides of
+ * a connection pointing at each other with inverse permutations, at least 7 nodes normal to a wall
+ * (CFD_E_TOPOLOGY otherwise).  `workspace` is device memory of at
  * least cfd_workspace_bytes(), caller-owned.  `cuda_stream` is a cudaStream_t (may be 0). */
 int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cfd_block_ptrs* ptrs, int nfaces,
                       const cfd_face* faces, const cfd_params* params, void* workspace, size_t workspace_bytes,
@@ -107,8 +113,9 @@ int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cf
  * Returns host values: synchronises the stream; CFD_E_JACOBIAN if J <= 0 at an interior node. */
 int cfd_compute_metrics(cfd_ctx*);
 
-/* S2 + S3 (Eqs. 9–19 with Steger–Warming splitting and the modified AFWENO of Fig. 11; Eqs. 5, 6, 21
- * with 6th-order central differences): r := J [ sum_d d(Fv^d)/d(xi^d) - sum_d D^d ] on interior points.
+/* S2 + S3 (Eqs. 9–19 with Steger–Warming splitting and the modified AFWENO of Fig. 11 -- or, with params.scheme = 1,
+ * the original ordering of Fig. 9; Eqs. 5, 6, 21 with 6th-order central differences, mu = 1 or Sutherland's mu(T)):
+ * r := J [ sum_d d(Fv^d)/d(xi^d) - sum_d D^d ] on interior points.
  * Requires valid ghost layers in q (cfd_exchange_interfaces + cfd_apply_bc).  Asynchronous. */
 int cfd_rhs(cfd_ctx*);
 
@@ -138,8 +145,7 @@ int cfd_cfl_dt(cfd_ctx*, double cfl, double* dt_host, double* const* dt_local_de
 /* Convenience: the four calls above for one stage, in Fig. 2's order, on the context's stream. */
 int cfd_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
 
-/* The same stage with the RK update fused into the last inviscid sweep (default sweep plan; other plans fall back
- * to cfd_stage): the zeta sweep forms R = J (r + X) point by point and writes a q^n + b (q + dt R) (Eq. 20) straight
+/* The same stage with the RK update fused into the last inviscid sweep: the zeta sweep forms R = J (r + X) point by point and writes a q^n + b (q + dt R) (Eq. 20) straight
  * into the r buffer, so R is never stored and no separate RK pass runs; stage 1 also reduces res_m = sum R_m^2
  * (fixed order).  Because q cannot be overwritten while neighbouring points still read it, the three state
  * buffers of every block EXCHANGE ROLES instead of being copied: after stage 1 the old r buffer holds q, the old
@@ -184,14 +190,17 @@ long long cfd_launch_count(const cfd_ctx*);
  * FMA = 2 flops) in *tflops; synchronises. */
 int cfd_fp64_peak_probe(int iters, double* tflops);
 
-/* Kernel plan of the three inviscid sweeps inside cfd_rhs (all plans compute the same R up to summation order):
- *   0 (default) all three as marching sweeps (one thread walks a grid line segment; every operand staged once per
- *     point through shared memory).  The xi sweep, whose lanes sit on lines a row pitch apart, is fed by TMA: boxes of
- *     4 positions x 32 lines per variable land swizzled in a per-warp ring and its output leaves by TMA stores
- *     (k_xi_tma); blocks with odd ni (row pitch not a multiple of 16 bytes) use a cp.async staging kernel instead;
- *   1 all three tiled (one thread per point);   2 all three with the plain marching kernel (the xi march reads with
- *     stride: for measurement);   3 xi tiled, eta and zeta marching;   4 plan 0 with the cp.async xi kernel forced.
- * cfd_stage_fused needs plan 0 or 4. */
+/* Kernel of the xi sweep inside cfd_rhs / cfd_stage_fused (all choices compute the same R up to summation order).
+ * All three sweeps are MARCHING sweeps (one thread walks a grid line segment; every operand staged once per point through
+ * shared memory); the xi sweep, whose lanes sit on lines a row pitch apart, runs out of a per-warp ring of 4-position
+ * chunks in shared memory:
+ *   0 (default)  ring filled by warp-cooperative 16-byte cp.async with a hand-made 32-byte swizzle, r written with 16-byte
+ *                stores (k_xi_ldg); blocks with odd ni (row pitch not a multiple of 16 bytes) use plan 4's kernel;
+ *   4            8-byte cp.async staging into padded per-line rings (k_march_xi), any ni;
+ *   5            ring filled by TMA boxes 4 x 32 x 1 x nvar with SWIZZLE_32B and written back by TMA stores (k_xi_tma;
+ *                correct, kept for measurement: the TMA unit is the bottleneck for 32-byte box rows); scheme 0 only.
+ * Other values (the tiled one-thread-per-point kernels of round 1, plans 1-3 and 6) are rejected with CFD_E_ARG: they were
+ * retired after profiles/r1_*.md settled the comparison. */
 int cfd_set_sweep_plan(cfd_ctx*, int plan);
 
 /* Device self-test of the branch-free fp64 reciprocal / reciprocal square root the hot kernels use instead

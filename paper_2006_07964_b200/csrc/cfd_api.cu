@@ -9,13 +9,13 @@ static thread_local std::string g_create_err;
 
 static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD_FACE_INTERFACE; }
 
-size_t ws_partials_offset_doubles(const cfd_ctx* c) { return (size_t)16 * (size_t)c->sum_M; }
+size_t ws_partials_offset_doubles(const cfd_ctx* c) { return (size_t)WS_ROWS * (size_t)c->sum_M; }
 int rk_max_partial_blocks() { return 16384; }
 
 extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
-  long long sum = 0;  // every block has its own 16 M doubles (the blocks' kernels run concurrently on side streams)
+  long long sum = 0;  // every block has its own WS_ROWS M doubles (the blocks' kernels run concurrently on side streams)
   for (int b = 0; b < nblocks; ++b) sum += (long long)(dims[b].ni + 2 * NG) * (dims[b].nj + 2 * NG) * (dims[b].nk + 2 * NG);
-  return ((size_t)16 * (size_t)sum + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
+  return ((size_t)WS_ROWS * (size_t)sum + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
 }
 
 // the six assignments of three buffers to the roles (q, qn, r): id -> role[]
@@ -160,10 +160,36 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
       for (int a = 0; a < 3; ++a)
         if (a != an && c->blk[F.nbr_block].n[F.perm[a]] != c->blk[F.block].n[a]) return bad("interface extents do not match");
     } else if (F.type == CFD_FACE_WALL_NOSLIP_ADIABATIC || F.type == CFD_FACE_FARFIELD_CHAR) {
+      // the wall closure reads the nodes 1..4 and mirrors the nodes 1..6 behind the wall: they must be interior nodes
+      if (F.type == CFD_FACE_WALL_NOSLIP_ADIABATIC && c->blk[F.block].n[F.face / 2] < NG + 1)
+        return bad("a wall needs at least 7 interior nodes along its normal");
       BcTask T{F.block, F.face, F.type};
       c->bcs.push_back(T);
     } else {
       return bad("unknown face type");
+    }
+  }
+  // every face of every block must be described (an undescribed face would leave its ghost layers unfilled), and
+  // the two sides of a connection must describe each other (U15)
+  for (int b = 0; b < nblocks; ++b)
+    for (int f = 0; f < 6; ++f)
+      if (!seen[(size_t)b * 6 + f]) {
+        delete c;
+        return fail_create(CFD_E_TOPOLOGY, "cfd_create_blocks: block " + std::to_string(b) + " face " + std::to_string(f) +
+                                               " has no face descriptor");
+      }
+  for (int t = 0; t < nfaces; ++t) {
+    const cfd_face& F = c->faces[t];
+    if (!is_connect(F.type)) continue;
+    const cfd_face* N = nullptr;
+    for (int u = 0; u < nfaces; ++u)
+      if (c->faces[u].block == F.nbr_block && c->faces[u].face == F.nbr_face) N = &c->faces[u];
+    bool ok = N && is_connect(N->type) && N->nbr_block == F.block && N->nbr_face == F.face;
+    for (int a = 0; ok && a < 3; ++a) ok = N->perm[F.perm[a]] == a && N->sign[F.perm[a]] == F.sign[a];  // inverse rotation
+    if (!ok) {
+      delete c;
+      return fail_create(CFD_E_TOPOLOGY, "cfd_create_blocks: face " + std::to_string(t) +
+                                             ": the neighbour's descriptor does not point back with the inverse permutation");
     }
   }
   // ---- workspace ----
@@ -176,7 +202,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   c->ws_bytes = workspace_bytes;
   {
     long long off = 0;
-    for (BlockDev& B : c->blk) { B.ws = c->ws + 16 * off; off += B.M; }
+    for (BlockDev& B : c->blk) { B.ws = c->ws + (long long)WS_ROWS * off; off += B.M; }
   }
   plan_copies(c);
   // ---- small device-side descriptor arrays (a few KB; the only allocations the library makes) ----
@@ -314,7 +340,6 @@ extern "C" int cfd_stage(cfd_ctx* c, int stage, double dt, double* res5) {
 extern "C" int cfd_stage_fused(cfd_ctx* c, int stage, double dt, double* res5) {
   if (!c) return CFD_E_ARG;
   if (stage < 1 || stage > 3) { c->err = "cfd_stage_fused: stage must be 1..3"; return CFD_E_STAGE; }
-  if (c->sweep_plan != 0) return cfd_stage(c, stage, dt, res5);  // only the default plan has the fused last sweep
   int rc = launch_rhs(c, stage, dt);
   if (rc != 0) return rc;
   // the new state was written to the r buffers: exchange the roles (stage 1: the old q becomes q^n, Eq. 20)
@@ -401,9 +426,7 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
 
 extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
   if (!c) return CFD_E_ARG;
-  if (plan < 0 || plan > 6) { c->err = "cfd_set_sweep_plan: plan must be 0..6"; return CFD_E_ARG; }
-  c->sweep_plan = plan >= 4 ? 0 : plan;
-  c->visc_tiled = plan == 6;
+  if (plan != 0 && plan != 4 && plan != 5) { c->err = "cfd_set_sweep_plan: plan must be 0, 4 or 5"; return CFD_E_ARG; }
   c->xi_mode = plan == 4 ? 2 : (plan == 5 ? 1 : 0);
   return CFD_OK;
 }

@@ -11,6 +11,10 @@
 
 #define NG CFD_NG
 
+// Scratch rows (doubles per stored point) of every block inside the caller's workspace: the viscous rows S (4), Fv^eta (4),
+// Fv^zeta (4); cfd_compute_metrics reuses them for the 9 first derivatives of the coordinates.
+constexpr int WS_ROWS = 12;
+
 // Device view of one block.  Strides in doubles: s[0] = 1, s[1] = m0, s[2] = m0*m1.
 struct BlockDev {
   int n[3];
@@ -18,7 +22,7 @@ struct BlockDev {
   long long M;
   long long s[3];
   double *q, *qn, *r, *xyz, *khat, *jac;
-  double* ws;  // this block's 16 M doubles of scratch inside the caller's workspace (viscous rows, phi / metric derivatives)
+  double* ws;  // this block's WS_ROWS M doubles of scratch inside the caller's workspace (viscous rows / metric derivatives)
   // offset of interior node (0,0,0)
   __host__ __device__ inline long long idx(int i, int j, int k) const {
     return ((long long)(k + NG) * m[1] + (j + NG)) * m[0] + (i + NG);
@@ -66,14 +70,12 @@ struct cfd_ctx {
   double* ws = nullptr;
   size_t ws_bytes = 0;
   long long max_M = 0;
-  long long sum_M = 0;                // sum of M over the blocks: the per-block scratch areas are 16 M doubles each
+  long long sum_M = 0;                // sum of M over the blocks: the per-block scratch areas are WS_ROWS M doubles each
   static constexpr int NSIDE = 4;     // side streams: the blocks of a multi-block case run their per-block kernels concurrently
   cudaStream_t side[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
   cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
   long long launches = 0;
-  int sweep_plan = 0;                 // cfd_set_sweep_plan
-  bool visc_tiled = false;            // cfd_set_sweep_plan(6): plan 0 with k_phi + k_visc_flux instead of k_visc_march
-  int xi_mode = 0;                    // plan 0 xi kernel: 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
+  int xi_mode = 0;                    // xi kernel (cfd_set_sweep_plan): 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
   std::string err;
   // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read
   bool prof_on = false;

@@ -2,6 +2,7 @@
 // and the FP64 peak probe.  sm_100a, fp64.  P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.
 #include "cfd_internal.cuh"
 #include "fastmath.cuh"
+#include "stencil.cuh"
 
 // =================================================================================================
 // S6: ghost fill through signed index permutations (U15; P:L262 bc_block, "on GPU without
@@ -13,8 +14,9 @@ __global__ void __launch_bounds__(256) k_fill(const CopyTask* __restrict__ tasks
   const long long cells = (long long)T.ext[0] * T.ext[1] * T.ext[2];
   const BlockDev D = blocks[T.dst_block];
   const BlockDev S = blocks[T.src_block];
-  double* __restrict__ dst = field == 0 ? D.q : D.xyz;
-  const double* __restrict__ src = field == 0 ? S.q : S.xyz;
+  // no __restrict__: for a self-periodic block dst and src are the same buffer (disjoint regions within a pass)
+  double* dst = field == 0 ? D.q : D.xyz;
+  const double* src = field == 0 ? S.q : S.xyz;
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < cells; t += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(t % T.ext[0]);
     const long long u = t / T.ext[0];
@@ -202,9 +204,6 @@ int launch_bc_q(cfd_ctx* c) {
 // Pass 1: xd[c*3+d] = d x_c / d xi^d into the workspace (valid where the index along d is in
 // [-3, n+3)); pass 2: khat on the box [-3, n+3)^3 from products, J from Eq. 8.
 // =================================================================================================
-__device__ __forceinline__ double d6(double m3, double m2, double m1, double p1, double p2, double p3) {
-  return (3.0 / 4.0) * (p1 - m1) - (3.0 / 20.0) * (p2 - m2) + (1.0 / 60.0) * (p3 - m3);
-}
 
 __global__ void __launch_bounds__(256) k_metric_d1(BlockDev B, double* __restrict__ xd) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -219,7 +218,7 @@ __global__ void __launch_bounds__(256) k_metric_d1(BlockDev B, double* __restric
     const long long st = B.s[d];
     for (int c = 0; c < 3; ++c) {
       const double* x = B.xyz + c * B.M + t;
-      xd[(c * 3 + d) * B.M + t] = d6(x[-3 * st], x[-2 * st], x[-st], x[st], x[2 * st], x[3 * st]);
+      xd[(c * 3 + d) * B.M + t] = d6c(x[-3 * st], x[-2 * st], x[-st], x[st], x[2 * st], x[3 * st]);
     }
   }
 }
@@ -241,9 +240,9 @@ __global__ void __launch_bounds__(256) k_metric_khat(BlockDev B, const double* _
       const double* a2 = xd + (c1 * 3 + d2) * M + p;
       const double* x2 = B.xyz + c2 * M + p;
       const long long S1 = B.s[d1], S2 = B.s[d2];
-      const double t1 = d6(a1[-3 * S2] * x2[-3 * S2], a1[-2 * S2] * x2[-2 * S2], a1[-S2] * x2[-S2], a1[S2] * x2[S2],
+      const double t1 = d6c(a1[-3 * S2] * x2[-3 * S2], a1[-2 * S2] * x2[-2 * S2], a1[-S2] * x2[-S2], a1[S2] * x2[S2],
                            a1[2 * S2] * x2[2 * S2], a1[3 * S2] * x2[3 * S2]);
-      const double t2 = d6(a2[-3 * S1] * x2[-3 * S1], a2[-2 * S1] * x2[-2 * S1], a2[-S1] * x2[-S1], a2[S1] * x2[S1],
+      const double t2 = d6c(a2[-3 * S1] * x2[-3 * S1], a2[-2 * S1] * x2[-2 * S1], a2[-S1] * x2[-S1], a2[S1] * x2[S1],
                            a2[2 * S1] * x2[2 * S1], a2[3 * S1] * x2[3 * S1]);
       B.khat[(d * 3 + c) * M + p] = t1 - t2;
     }

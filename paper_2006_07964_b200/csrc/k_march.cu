@@ -17,6 +17,7 @@
 #include "cfd_internal.cuh"
 #include "sweep_math.cuh"
 #include "march_fir.cuh"
+#include "stencil.cuh"
 #include <cmath>
 
 namespace {
@@ -34,7 +35,7 @@ struct MarchArgs {
   const double* W;      // viscous flux rows of direction d, + interior origin (VISC)
   const double* jac;    // + interior origin (ACC 2)
   const double* qn;     // q^n + interior origin (ACC 3, stages 2 and 3)
-  const double* Sx;     // SX: S = d(Fv^xi)/d(xi) rows 2..5 (k_visc_flux<true>), + interior origin
+  const double* Sx;     // SX: S = d(Fv^xi)/d(xi) rows 2..5 (k_visc_march), + interior origin
   double* r;            // + interior origin
   double* partials;     // ACC 3 stage 1: 5 partial sums of R_m^2 per CTA
   long long M;          // plane stride between variables
@@ -43,14 +44,6 @@ struct MarchArgs {
   double gamma, eps4;
   double dt, rk_a, rk_b; // ACC 3 (Eq. 20)
 };
-
-__device__ __forceinline__ void cp8(double* dst, const double* src) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ACC 0: r = X;  1: r += X;  2: r = J (r + X);  3: the RK stage fused into the last sweep (Eq. 20):
 //   with R = J (r + X):  out = a q^n + b (q + dt R)  written to the r buffer (the caller then exchanges the roles of the
@@ -74,7 +67,7 @@ constexpr int march_smem_doubles() {
   return (RING * RV + (VISC ? 8 : 0) + 2 * OutCfg<ACC, ST1, SX>::NOUT + ((ACC == 3 && ST1) ? 5 : 0)) * MT;
 }
 
-// SX (with ACC >= 1): the viscous xi term S written by k_visc_flux<true> is added to r here (the xi sweep runs first
+// SX (with ACC >= 1): the viscous xi term S written by k_visc_march is added to r here (the xi sweep runs first
 // and knows nothing about viscosity).
 // SCH: 0 = modified AFWENO (Fig. 11: eigen-system at the point, shared beta), 1 = original AFWENO (Fig. 9, NEXT-1:
 // eigen-system at the interface, two complete interpolations over j-3 .. j+2; sweep_math.cuh afweno_iface_orig).
@@ -286,9 +279,6 @@ constexpr int XWARPS = 4;
 struct XiArgs {
   const double* q;      // + interior origin
   const double* kh;
-  const double* W;      // unused (the viscous xi rows never reach this kernel)
-  const double* Sx;     // VISC: S = d(Fv^xi)/d(xi) rows 2..5 from k_visc_flux<true>, added to r in the flush
-  const double* jac;
   double* r;
   long long M;          // plane stride between variables
   long long sl, st;     // strides: neighbouring line (lane axis), third index; the sweep runs along stride 1
@@ -300,7 +290,6 @@ struct XiArgs {
 
 __device__ __forceinline__ int wrap10(int s) { return s >= XR ? s - XR : s; }
 
-template <int ACC, bool VISC>
 __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
   extern __shared__ double ring[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -355,15 +344,8 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
         if (!lok[t]) continue;
         const double* sX = lbase + t * 8 * XLS + s;
         double* gr = A.r + goff[t] + pos;
-        double jac = 0.0;
-        if (ACC == 2) jac = A.jac[goff[t] + pos];
 #pragma unroll
-        for (int m = 0; m < 5; ++m) {
-          double X = sX[m * XR];
-          if (ACC == 0) gr[m * M] = X;
-          else if (ACC == 1) gr[m * M] = gr[m * M] + X;
-          else gr[m * M] = jac * (gr[m * M] + X);
-        }
+        for (int m = 0; m < 5; ++m) gr[m * M] = sX[m * XR];
       }
     }
   };
@@ -458,15 +440,6 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
   }
 }
 
-template <int ACC>
-void launch_march_xi_t(cfd_ctx* c, const XiArgs& A, bool visc) {
-  const long long units = (long long)A.nlb * A.nt;
-  dim3 grid((unsigned)((units + XWARPS - 1) / XWARPS), (unsigned)((A.n + A.S - 1) / A.S));
-  const size_t smem = sizeof(double) * XWARPS * 32 * XLS;
-  if (visc) k_march_xi<ACC, true><<<grid, 32 * XWARPS, smem, c->stream>>>(A);
-  else k_march_xi<ACC, false><<<grid, 32 * XWARPS, smem, c->stream>>>(A);
-}
-
 }  // namespace
 
 // Segment count along the sweep: enough CTAs to fill 148 SMs x 2 resident CTAs, as few partial waves as possible,
@@ -510,9 +483,10 @@ int march_init() {
 #define OPT(A, S)                                          \
   if (e == cudaSuccess) e = march_attr<A, true, S>();      \
   if (e == cudaSuccess) e = march_attr<A, false, S>();
-  OPT(0, false) OPT(1, false) OPT(2, false) OPT(3, false) OPT(3, true)
+  OPT(2, false) OPT(3, false) OPT(3, true)
 #undef OPT
   if (e == cudaSuccess) e = march_attr<1, true, false, true>();
+  if (e == cudaSuccess) e = march_attr<1, false, false, false>();
   // scheme 1 (original AFWENO): the kernels of the default plan only
   if (e == cudaSuccess) e = march_attr<0, false, false, false, 1>();
   if (e == cudaSuccess) e = march_attr<1, true, false, true, 1>();
@@ -523,11 +497,7 @@ int march_init() {
   OPT1(2, false) OPT1(3, false) OPT1(3, true)
 #undef OPT1
   const int smx = (int)(sizeof(double) * XWARPS * 32 * XLS);
-#define OPTX(A)                                                                                                        \
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi<A, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx); \
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi<A, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
-  OPTX(0) OPTX(1) OPTX(2)
-#undef OPTX
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_march_xi, cudaFuncAttributeMaxDynamicSharedMemorySize, smx);
   return e == cudaSuccess ? 0 : -1;
 }
 
@@ -582,26 +552,22 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
     else GO1(2, false);
   }
   else if (rk) { if (rk->stage == 1) GO(3, true); else GO(3, false); }
-  else if (acc == 0) GO(0, false);
   else if (acc == 1 && sx && visc) launch_march_k<1, true, false, true>(c, A);
-  else if (acc == 1) GO(1, false);
-  else GO(2, false);
+  else if (acc == 1 && !visc) launch_march_k<1, false, false, false>(c, A);
+  else if (acc == 2) GO(2, false);
+  else { c->err = "launch_march: this accumulation mode is not instantiated"; return CFD_E_ARG; }
 #undef GO
 #undef GO1
   c->launches++;
   return 0;
 }
 
-// The xi sweep of block B as a staged marching sweep (k_march_xi) with accumulation mode acc.
-int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
-  const bool visc = false;  // the viscous xi term S is added by the eta sweep
+// The xi sweep of block B (r = X^xi) as a staged marching sweep (k_march_xi): blocks with odd ni and plan 4.
+int launch_march_xi(cfd_ctx* c, const BlockDev& B) {
   const long long o0 = B.idx(0, 0, 0);
   XiArgs A;
   A.q = B.q + o0;
   A.kh = B.khat + o0;
-  A.W = nullptr;
-  A.Sx = visc ? B.ws + o0 : nullptr;
-  A.jac = B.jac + o0;
   A.r = B.r + o0;
   A.M = B.M;
   A.sl = B.s[1]; A.st = B.s[2];
@@ -613,9 +579,8 @@ int launch_march_xi(cfd_ctx* c, const BlockDev& B, int acc) {
   A.S = (A.n + nseg - 1) / nseg;
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;
-  if (acc == 0) launch_march_xi_t<0>(c, A, visc);
-  else if (acc == 1) launch_march_xi_t<1>(c, A, visc);
-  else launch_march_xi_t<2>(c, A, visc);
+  dim3 grid((unsigned)((units + XWARPS - 1) / XWARPS), (unsigned)((A.n + A.S - 1) / A.S));
+  k_march_xi<<<grid, 32 * XWARPS, sizeof(double) * XWARPS * 32 * XLS, c->stream>>>(A);
   c->launches++;
   return 0;
 }

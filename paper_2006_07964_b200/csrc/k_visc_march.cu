@@ -15,6 +15,7 @@
 // W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).  Same arithmetic per point as k_phi + k_visc_flux.
 #include "cfd_internal.cuh"
 #include "fastmath.cuh"
+#include "stencil.cuh"
 #include <cmath>
 
 namespace {
@@ -37,13 +38,6 @@ struct VG {
   static constexpr int SMEM = (SM_PHI + SM_WX + SM_Q + SM_H) * 8;
 };
 
-__device__ __forceinline__ void vcp8(double* dst, const double* src) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src) : "memory");
-}
-__device__ __forceinline__ double vd6c(double m3, double m2, double m1, double p1, double p2, double p3) {
-  return (3.0 / 4.0) * (p1 - m1) - (3.0 / 20.0) * (p2 - m2) + (1.0 / 60.0) * (p3 - m3);
-}
 // phi = (u, v, w, T = gamma p / rho) from the conservative state: the arithmetic of k_phi
 __device__ __forceinline__ void phi_of(double r, double m1, double m2, double m3, double e, double gamma, double f[4]) {
   const double ir = frcp(r);
@@ -98,17 +92,17 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
     if (col_in && k + 3 + NG < B.m[2]) {
       const long long o = pcol + (long long)(k + 3 + NG) * s2;
 #pragma unroll
-      for (int m = 0; m < 5; ++m) vcp8(sq + m * NT + tid, B.q + m * M + o);
+      for (int m = 0; m < 5; ++m) cp8(sq + m * NT + tid, B.q + m * M + o);
     }
 #pragma unroll
     for (int h = 0; h < HPT; ++h) {
       if (halo_in[h]) {
         const long long o = phal[h] + (long long)(k + NG) * s2;
 #pragma unroll
-        for (int m = 0; m < 5; ++m) vcp8(sh + (m * HPT + h) * NT + tid, B.q + m * M + o);
+        for (int m = 0; m < 5; ++m) cp8(sh + (m * HPT + h) * NT + tid, B.q + m * M + o);
       }
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    cp_commit();
   };
 
   // ---- prologue: phi of my column at kb-3 .. kb+2 ----
@@ -133,12 +127,12 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
 #pragma unroll
       for (int m = 0; m < 4; ++m) {
         const double* a = sx + (m * VY + ty) * VX + tx;
-        W[(long long)m * M + p] = vd6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
+        W[(long long)m * M + p] = d6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
       }
     }
   };
   for (int k = kb; k < ke; ++k) {
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    cp_wait<0>();
     const bool ok = k < 0 || k >= B.n[2];
     double* const pl = sphi + (k & 1) * (4 * PR * PC);
     // ---- newest plane of my column into the register pipeline; plane k (my own phi and my halo cell) into shared memory ----
@@ -177,9 +171,9 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
 #pragma unroll
       for (int f = 0; f < 4; ++f) {
         const double* a = pl + (f * PR + ty + 3) * PC + tx + 3;
-        const double dx = vd6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
-        const double dy = vd6c(a[-3 * PC], a[-2 * PC], a[-PC], a[PC], a[2 * PC], a[3 * PC]);
-        const double dz = vd6c(ph[0][f], ph[1][f], ph[2][f], ph[4][f], ph[5][f], ph[6][f]);
+        const double dx = d6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
+        const double dy = d6c(a[-3 * PC], a[-2 * PC], a[-PC], a[PC], a[2 * PC], a[3 * PC]);
+        const double dz = d6c(ph[0][f], ph[1][f], ph[2][f], ph[4][f], ph[5][f], ph[6][f]);
 #pragma unroll
         for (int c = 0; c < 3; ++c) g[c][f] = J * ((kh[0][c] * dx + kh[1][c] * dy) + kh[2][c] * dz);
       }

@@ -17,7 +17,6 @@
 //                       unit needs ~5 cycles per 32-byte box row on B200, which makes this variant TMA-bound.
 // Array index along i: a = position + NG; chunks are a/4, so r groups are aligned for NG = 6 ((NG-2) % 4 == 0) when
 // segments start at multiples of 4.  The xi sweep runs first (r = X); the viscous xi term S is added by the eta sweep.
-// (The VISC template parameter / the S buffer of the ring are the earlier variant in which the flush added S; unused.)
 #include <cuda.h>
 
 #include "cfd_internal.cuh"
@@ -31,9 +30,9 @@ namespace {
 constexpr int TW = 4;                       // warps per CTA
 constexpr int PLANE = 32 * 32;              // bytes of one variable of one chunk: 32 lines x 32 B
 constexpr int SLOT = 8 * PLANE;             // Q (5) + khat (3)
-constexpr int WARP_BYTES = 3 * SLOT + 4 * PLANE;  // ring of 3 chunks + S buffer (4 rows) = 28 KB
+constexpr int WARP_BYTES = 3 * SLOT;         // ring of 3 chunks = 24 KB
 constexpr int XT_SMEM = TW * WARP_BYTES + 256 /*alignment slack*/ + TW * 4 * 8 /*mbarriers*/;
-constexpr int XL_SMEM = TW * 3 * SLOT + 256;  // k_xi_ldg: ring only
+constexpr int XL_SMEM = TW * WARP_BYTES + 256;  // k_xi_ldg: no mbarriers
 
 struct XiTArgs {
   int nl, nt, n, S;     // lines (j), third extent (k), sweep length, segment length (multiple of 4)
@@ -162,11 +161,10 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
   }
 }
 
-// VISC: the flush adds S = d(Fv^xi)/d(xi) (rows 2..5) before the store.   r = X (+ S); the xi sweep runs first.
-template <bool VISC>
+// r = X^xi; the xi sweep runs first and carries no viscous data (the eta sweep adds S = d(Fv^xi)/d(xi)).
 __global__ void __launch_bounds__(32 * TW, 2)
 k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtensorMap tk, const __grid_constant__ CUtensorMap tr,
-         const __grid_constant__ CUtensorMap ts, XiTArgs A) {
+         XiTArgs A) {
   extern __shared__ char smem_raw[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const long long unit = (long long)blockIdx.x * TW + wid;
@@ -175,11 +173,10 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
   if (it >= A.nt) return;  // warp-uniform; the kernel has no CTA-wide barrier
   const int p0 = blockIdx.y * A.S;  // multiple of 4
   const int p1 = min(A.n, p0 + A.S);
-  // shared memory: [TW] x (3 chunk slots + S buffer), 256-byte aligned (the swizzle uses address bits 4 and 7)
+  // shared memory: [TW] x 3 chunk slots, 256-byte aligned (the swizzle uses address bits 4 and 7)
   char* const base = smem_raw + ((256u - (smem_u32(smem_raw) & 255u)) & 255u);
   char* const ring = base + wid * WARP_BYTES;
-  char* const sxbuf = ring + 3 * SLOT;
-  const unsigned bars = smem_u32(base + TW * WARP_BYTES) + wid * 32;  // full[0..2], sx
+  const unsigned bars = smem_u32(base + TW * WARP_BYTES) + wid * 32;  // full[0..2]
   const int c1 = lb * 32 + NG, c2 = it + NG;  // TMA coordinates of this warp's first line
   const int swz = (lane >> 2) & 1;
   const int off0 = lane * 32 + (swz << 4), off1 = lane * 32 + ((swz ^ 1) << 4);  // pair 0 / 1 of my line inside a plane
@@ -194,34 +191,15 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
     tma_load4(dst, &tq, bar, ch * 4, c1, c2, 0);
     tma_load4(dst + 5 * PLANE, &tk, bar, ch * 4, c1, c2, 0);
   };
-  auto load_sx = [&](int ch) {  // lane 0 only
-    mbar_expect_tx(bars + 24, 4 * PLANE);
-    tma_load4(smem_u32(sxbuf), &ts, bars + 24, ch * 4, c1, c2, 0);
-  };
-  unsigned par_full = 0, par_sx = 0;  // phase parity to wait for, per barrier
+  unsigned par_full = 0;  // phase parity to wait for, per barrier
   auto wait_chunk = [&](int ch) {
     const int s = ch % 3;
     mbar_wait(bars + s * 8, (par_full >> s) & 1u);
     par_full ^= 1u << s;
   };
-  // r positions 4(ch-1) .. 4(ch-1)+3 are parked in the Q planes of chunk ch: add S, store the box, free the slot
+  // r positions 4(ch-1) .. 4(ch-1)+3 are parked in the Q planes of chunk ch: store the box, free the slot
   auto flush = [&](int ch) {
     char* const slot = ring + (ch % 3) * SLOT;
-    if (VISC) {
-      mbar_wait(bars + 24, par_sx);
-      par_sx ^= 1u;
-#pragma unroll
-      for (int m = 1; m < 5; ++m) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          double2* x = reinterpret_cast<double2*>(slot + m * PLANE + (h ? off1 : off0));
-          const double2 sv = *reinterpret_cast<const double2*>(sxbuf + (m - 1) * PLANE + (h ? off1 : off0));
-          double2 v = *x;
-          v.x += sv.x; v.y += sv.y;
-          *x = v;
-        }
-      }
-    }
     fence_async();
     __syncwarp();
     if (lane == 0) {
@@ -231,7 +209,7 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
   };
 
   if (lane == 0) {
-    for (int b = 0; b < 4; ++b) mbar_init(bars + b * 8, 1);
+    for (int b = 0; b < 3; ++b) mbar_init(bars + b * 8, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_async();
   }
@@ -280,14 +258,13 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
     }
     xi_step<1>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4);
     if (ev) {
-      // refill the freed slot with the chunk two ahead (if any step will read it) and fetch S for the chunk being
-      // parked now; the TMA store issued by flush() must have finished reading the slot first
+      // refill the freed slot with the chunk two ahead (if any step will read it); the TMA store issued by flush() must
+      // have finished reading the slot first
       __syncwarp();
       if (lane == 0) {
         tma_wait_read0();
         const int cn = (a >> 2) + 2;
         if (cn * 4 <= p1 + NG + 2) load_chunk(cn);
-        if (VISC) load_sx(a >> 2);
       }
     }
     // ---------------- step B (a + 1 even) ----------------
@@ -335,7 +312,7 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
   const int p0 = blockIdx.y * A.S;  // multiple of 4
   const int p1 = min(A.n, p0 + A.S);
   char* const base = smem_raw + ((256u - (smem_u32(smem_raw) & 255u)) & 255u);
-  char* const ring = base + wid * (3 * SLOT);
+  char* const ring = base + wid * WARP_BYTES;
   const int swz = (lane >> 2) & 1;
   const int off0 = lane * 32 + (swz << 4), off1 = lane * 32 + ((swz ^ 1) << 4);
   auto pair_ptr = [&](int pn) -> char* { return ring + ((pn >> 1) % 3) * SLOT + ((pn & 1) ? off1 : off0); };
@@ -453,7 +430,6 @@ struct XiMaps {
   bool ok = false;
   CUtensorMap st[3];  // the caller's q, qn, r buffers (cfd_ctx::base): 4-D (i, j, k, var), box 4 x 32 x 1 x 5
   CUtensorMap kh;     // khat^xi rows: box 4 x 32 x 1 x 3
-  CUtensorMap sx;     // S rows in the workspace: box 4 x 32 x 1 x 4
 };
 struct XiTmaState {
   std::vector<XiMaps> maps;
@@ -476,7 +452,7 @@ bool encode(EncodeTiledFn fn, CUtensorMap* tm, const BlockDev& B, double* basep,
 }  // namespace
 
 // Builds the tensor maps of every block whose layout TMA accepts (row pitch a multiple of 16 bytes, i.e. ni even).
-// Blocks without maps use the cp.async xi kernel (k_march_xi) instead.  Never fails: "no TMA" is a valid outcome.
+// Blocks without maps use the 16-byte cp.async ring kernel (k_xi_ldg) or, for odd ni, k_march_xi instead.  Never fails: "no TMA" is a valid outcome.
 void xi_tma_setup(cfd_ctx* c) {
   XiTmaState* S = new XiTmaState;
   S->maps.resize(c->blk.size());
@@ -494,8 +470,7 @@ void xi_tma_setup(cfd_ctx* c) {
     cudaGetLastError();
     return;
   }
-  if (cudaFuncSetAttribute(k_xi_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess ||
-      cudaFuncSetAttribute(k_xi_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess) {
+  if (cudaFuncSetAttribute(k_xi_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, XT_SMEM) != cudaSuccess) {
     cudaGetLastError();
     return;
   }
@@ -506,7 +481,6 @@ void xi_tma_setup(cfd_ctx* c) {
     bool ok = true;
     for (int t = 0; t < 3; ++t) ok = ok && encode(fn, &X.st[t], B, c->base[t][b], 5);
     ok = ok && encode(fn, &X.kh, B, B.khat, 3);
-    ok = ok && encode(fn, &X.sx, B, B.ws, 4);
     X.ok = ok;
   }
 }
@@ -528,7 +502,7 @@ bool xi_ldg_ok(const cfd_ctx* c, int b) {
 
 int pick_segments(long long ctas_per_seg, int n, int quantum);
 
-// The xi sweep of block b (r = X + S) with the chunk-ring marching kernel; tma: fill the ring by TMA (k_xi_tma),
+// The xi sweep of block b (r = X^xi) with the chunk-ring marching kernel; tma: fill the ring by TMA (k_xi_tma),
 // else by 16-byte cp.async (k_xi_ldg, the default: the TMA unit is the bottleneck for 32-byte box rows).
 int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
   const XiTmaState* S = static_cast<const XiTmaState*>(c->xi_tma);
@@ -556,7 +530,7 @@ int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
   }
   const CUtensorMap& tq = X.st[c->role[0]];
   const CUtensorMap& tr = X.st[c->role[2]];
-  k_xi_tma<false><<<grid, 32 * TW, XT_SMEM, c->stream>>>(tq, X.kh, tr, X.sx, A);  // S is added by the eta sweep
+  k_xi_tma<<<grid, 32 * TW, XT_SMEM, c->stream>>>(tq, X.kh, tr, A);
   c->launches++;
   return 0;
 }

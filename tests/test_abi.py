@@ -40,9 +40,9 @@ def test_workspace_bytes_is_pure_host_arithmetic(lib):
     d = (lib._Dims * 2)(lib._Dims(32, 32, 32), lib._Dims(10, 20, 30))
     p = lib._Params()
     got = lib.lib.cfd_workspace_bytes(2, d, C.byref(p))
-    M = 44 ** 3 + 22 * 32 * 42  # every block has its own 16 M doubles of scratch (blocks run concurrently)
-    assert got >= 16 * M * 8
-    assert got < 16 * M * 8 + 2 * 16384 * 5 * 8 + (1 << 12)  # + residual partials (16384 CTAs x 5 per block)
+    M = 44 ** 3 + 22 * 32 * 42  # every block has its own 12 M doubles of scratch (blocks run concurrently)
+    assert got >= 12 * M * 8
+    assert got < 12 * M * 8 + 2 * 16384 * 5 * 8 + (1 << 12)  # + residual partials (16384 CTAs x 5 per block)
 
 
 def test_no_cuda_device_fails_loudly(lib):

@@ -126,13 +126,14 @@ def test_rhs_parity(po, W, B, which):
     assert_rhs_parity(o, g, case)
 
 
-@pytest.mark.parametrize("plan", [1, 2, 3, 4, 5, 6])
-@pytest.mark.parametrize("which", ["ragged-ns", "ragged-euler", "multiblock-ns", "cylinder-ns", "tiny"])
+@pytest.mark.parametrize("plan", [4, 5])
+@pytest.mark.parametrize("which", ["ragged-ns", "ragged-euler", "ragged-even-ns", "multiblock-ns", "cylinder-ns", "tiny"])
 def test_rhs_parity_other_sweep_plans(po, W, B, which, plan):
-    """cfd_set_sweep_plan: all-tiled (1), all k_march (2), xi tiled + marching (3) and the default plan with the
-    cp.async xi kernel forced (4) against the oracle (plan 0 is the default everywhere else)."""
+    """cfd_set_sweep_plan: the xi sweep with the 8-byte cp.async staging kernel forced (4) and with the TMA-fed chunk
+    ring (5) against the oracle (plan 0, the 16-byte cp.async chunk ring, is the default everywhere else)."""
     case = {"ragged-ns": lambda: ragged_case(W, 1),
             "ragged-euler": lambda: ragged_case(W, 0),
+            "ragged-even-ns": lambda: ragged_case(W, 1, n=(70, 45, 9)),
             "multiblock-ns": lambda: W.c4_multiblock(nb=12, mach=0.3),
             "cylinder-ns": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0, noise=1e-2),
             "tiny": lambda: W.tgv_sine_box(6, viscous=1, mach=0.3)}[which]()
@@ -180,9 +181,8 @@ def test_scheme1_fused_steps_match_oracle(po, W, B):
     assert np.allclose(rg, ro, rtol=1e-10)
     qo, qg = o.interior(0, "q"), g.to_numpy(0, "q")
     assert np.abs(qg - qo).max() < 1e-12 * np.abs(qo).max()
-    g.set_sweep_plan(1)
-    with pytest.raises(B.CfdError):  # the tiled plans do not implement scheme 1
-        g.rhs()
+    with pytest.raises(B.CfdError):  # plans 1-3 and 6 (tiled kernels) were retired in round 2
+        g.set_sweep_plan(1)
 
 
 def noisy_vortex_case(W):
@@ -456,6 +456,21 @@ def test_error_codes(W, B):
     with pytest.raises(B.CfdError) as e:
         B.Context([(4, 8, 8)], [], case.params)
     assert e.value.code == -1
+    missing = [dict(f) for f in case.faces][:-1]  # one face without a descriptor
+    with pytest.raises(B.CfdError) as e:
+        B.Context(case.dims, missing, case.params)
+    assert e.value.code == -2
+    oneway = [dict(f) for f in case.faces]
+    oneway[0]["nbr_face"], oneway[0]["type"] = oneway[0]["nbr_face"], W.INTERFACE
+    oneway[1]["nbr_block"] = 0
+    oneway[1]["nbr_face"] = oneway[1]["face"]  # points at itself instead of back at face 0
+    with pytest.raises(B.CfdError) as e:
+        B.Context(case.dims, oneway, case.params)
+    assert e.value.code == -2
+    thin = W.c5_cylinder(ni=16, nj=6, nk=8, ratio=1.3, r_out=4.0)  # 6 nodes normal to the wall: the mirror would read a ghost
+    with pytest.raises(B.CfdError) as e:
+        B.Context(thin.dims, thin.faces, thin.params)
+    assert e.value.code == -2
     # left-handed grid -> J < 0
     flipped = W.c1_vortex(8)
     flipped.xyz[0] = flipped.xyz[0][:, :, :, ::-1].copy()
@@ -552,17 +567,14 @@ def test_cfl_dt_matches_oracle(po, W, B, which):
 # ------------------------------------------------------------------------------------------------
 # NEXT-3: Sutherland viscosity mu(T) and a shocked workload (shock-vortex slab on the seeded wavy periodic grid)
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("which", ["tgv-sutherland", "ragged-sutherland", "cylinder-sutherland", "ragged-sutherland-plan6"])
+@pytest.mark.parametrize("which", ["tgv-sutherland", "ragged-sutherland", "cylinder-sutherland"])
 def test_rhs_parity_sutherland(po, W, B, which):
     case = {"tgv-sutherland": lambda: W.tgv_sine_box(24, viscous=1, mach=0.4),
             "ragged-sutherland": lambda: ragged_case(W, 1),
-            "ragged-sutherland-plan6": lambda: ragged_case(W, 1),
             "cylinder-sutherland": lambda: W.c5_cylinder(ni=64, nj=24, nk=10, ratio=1.15, r_out=10.0, noise=1e-2)}[which]()
     case.params["sutherland"] = 110.4 / 288.15
     case.params["reynolds"] = 50.0   # viscous terms large enough that mu(T) matters at the 1e-12 level
     o, g = pair(po, B, case)
-    if which.endswith("plan6"):
-        g.set_sweep_plan(6)
     assert_rhs_parity(o, g, case)
     if not which.startswith("ragged"):
         return  # T = 1 in the TGV field, ~1 around the cylinder: mu(T) ~ 1 there; the ragged field has T varying by 25 %
