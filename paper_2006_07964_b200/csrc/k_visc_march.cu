@@ -8,8 +8,8 @@
 //   * the (i, j) plane of phi at k (tile + halo of 3 in j, 6 in i) lives in SHARED memory, double buffered: the xi and
 //     eta stencils read it with LDS;
 //   * Q of plane k+4 and the halo cells of plane k+1 arrive by cp.async in thread-private shared-memory slots one step
-//     ahead (no registers held across a step); the ten metric values are loaded before the plane barrier and used
-//     after it (staging them through shared memory as well cost more shared-memory instructions than it hid latency);
+//     ahead (no registers held across a step); the ten metric values of plane k+1 are loaded at the end of step k, when few
+//     registers are live (staging them through shared memory cost more shared-memory instructions than it hid latency);
 //   * the xi rows of the flux go to shared memory and come back as S = d(Fv^xi)/d(xi), as in k_visc_flux<true>.
 // Output (workspace rows): W[0..3] = S on interior points; W[4..7] = Fv^eta rows 2..5 on (i, k) interior, j in [-3, nj+3);
 // W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).  Same arithmetic per point as k_phi + k_visc_flux.
@@ -119,6 +119,24 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
     }
   }
   stage(kb);
+  // the ten metric values of plane k are loaded at the END of step k-1 (after its flux arithmetic, when few registers are
+  // live) and used in the second half of step k: half a step of distance covers the DRAM latency of these streaming loads
+  double kh[3][3], J = 0.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) kh[d][c] = 0.0;
+  auto load_metrics = [&](int k) {
+    if (any) {
+      const long long o = pcol + (long long)(k + NG) * s2;
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) kh[d][c] = __ldg(B.khat + (d * 3 + c) * M + o);
+      J = __ldg(B.jac + o);
+    }
+  };
+  load_metrics(kb);
   const double mu0 = P.mu, kap0 = P.kappa, suth = P.suth;
   auto s_of_plane = [&](int kk) {
     if (own && !oj && col_in && kk >= 0 && kk < B.n[2]) {
@@ -149,15 +167,6 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
 #pragma unroll
         for (int f = 0; f < 4; ++f) pl[f * PR * PC + hpl[h]] = hf[f];
       }
-    }
-    double kh[3][3], J = 0.0;
-    if (any) {
-      const long long o = pcol + (long long)(k + NG) * s2;
-#pragma unroll
-      for (int d = 0; d < 3; ++d)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) kh[d][c] = __ldg(B.khat + (d * 3 + c) * M + o);
-      J = __ldg(B.jac + o);
     }
     if (k + 1 < ke) stage(k + 1);
     __syncthreads();
@@ -213,6 +222,7 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
         }
       }
     }
+    if (k + 1 < ke) load_metrics(k + 1);
 #pragma unroll
     for (int t = 0; t < 6; ++t)
 #pragma unroll
