@@ -8,15 +8,19 @@
 // reads "my line, positions (2h, 2h+1)" of a quarter warp hit 8 distinct bank groups: conflict-free LDS.128.
 // Nothing crosses warps: __syncwarp (and warp-private mbarriers in the TMA variant) only.
 //   * step j reads Q at j-2..j+2 and khat at j-3..j+2 as 3-4 position pairs and computes exactly what k_march does;
-//   * the output of step j (r at position j-1) is parked in the Q words of position j-3 (dead: Q is read at j-2..j+2
-//     only), i.e. r positions 4g-4..4g-1 fill exactly one chunk; when that chunk's last park is done it is written to r
-//     in full sectors and the freed slot is refilled with the chunk two ahead.
+//   * the output of step j (r at position j-1, array index x = j+5) is parked in shared memory and leaves in groups of
+//     four positions per line.  k_xi_ldg writes SECTOR-ALIGNED groups (array indices 4c..4c+3: x = 4c, 4c+1 wait in a
+//     2.5 KB side buffer, x = 4c+2, 4c+3 in the dead Q words of positions 4c, 4c+1); k_xi_tma stores the box of a whole
+//     chunk (x = 4c+2..4c+5 parked in the Q words of chunk c), which straddles two half sectors per line because
+//     interior position 0 sits at array index NG = 6, 16 bytes into a sector.  When a chunk's khat has been read for
+//     the last time its slot is refilled with the chunk two ahead.
 // Two ways to fill the ring and to write r:
-//   k_xi_ldg (default)  warp-cooperative 16-byte cp.async (lane -> line l/2 + 16t, half l%2), swizzle by hand, STG.128;
+//   k_xi_ldg (default)  warp-cooperative 16-byte cp.async (lane -> line l/2 + 16t, half l%2), swizzle by hand, STG.128 of
+//                       full sectors;
 //   k_xi_tma (plan 5)   cp.async.bulk.tensor boxes 4 x 32 x 1 x nvar with SWIZZLE_32B, TMA store; correct, but the TMA
 //                       unit needs ~5 cycles per 32-byte box row on B200, which makes this variant TMA-bound.
-// Array index along i: a = position + NG; chunks are a/4, so r groups are aligned for NG = 6 ((NG-2) % 4 == 0) when
-// segments start at multiples of 4.  The xi sweep runs first (r = X); the viscous xi term S is added by the eta sweep.
+// Array index along i: a = position + NG; chunks are a/4; segments start at multiples of 4 (interior), so a segment's
+// first and last output group are half groups (masked stores).  The xi sweep runs first (r = X); the viscous xi term S is added by the eta sweep.
 #include <cuda.h>
 
 #include "cfd_internal.cuh"
@@ -32,7 +36,8 @@ constexpr int PLANE = 32 * 32;              // bytes of one variable of one chun
 constexpr int SLOT = 8 * PLANE;             // Q (5) + khat (3)
 constexpr int WARP_BYTES = 3 * SLOT;         // ring of 3 chunks = 24 KB
 constexpr int XT_SMEM = TW * WARP_BYTES + 256 /*alignment slack*/ + TW * 4 * 8 /*mbarriers*/;
-constexpr int XL_SMEM = TW * WARP_BYTES + 256;  // k_xi_ldg: no mbarriers
+constexpr int XL_WARP_BYTES = 3 * SLOT + 5 * 512;   // k_xi_ldg: ring + side buffer of parked outputs (2.5 KB)
+constexpr int XL_SMEM = TW * XL_WARP_BYTES + 256;
 
 struct XiTArgs {
   int nl, nt, n, S;     // lines (j), third extent (k), sweep length, segment length (multiple of 4)
@@ -89,9 +94,10 @@ struct XiState {
 #define LD2(P, v) (*reinterpret_cast<const double2*>((P) + (v) * PLANE))
 // SCH 0: modified AFWENO (eigen-system at point a, Fig. 11); SCH 1: original AFWENO (eigen-system at interface a-1/2,
 // two complete interpolations over a-3 .. a+2, Fig. 9; NEXT-1).
+// park / pstr: where the output of this step (r at array index a-1) is parked: park[m * pstr], m = 0..4.
 template <int PAR, int SCH = 0>
 __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, const char* P2, const char* P3, bool iface, bool store,
-                                        double gamma, double eps4) {
+                                        double gamma, double eps4, double* park, int pstr) {
   double Qs[5][5], UL[5], UR[5], Fc[5];
 #pragma unroll
   for (int m = 0; m < 5; ++m) {
@@ -147,11 +153,10 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
       sw_flux<+1>(UL, kh[0], kh[1], kh[2], kn, ikn, gamma, Fp);
       sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Fm);
     }
-    double* park = reinterpret_cast<double*>(P0) + (PAR ? 0 : 1);  // the Q words of position a-3
 #pragma unroll
     for (int m = 0; m < 5; ++m) {
       const double Phi = (Fp[m] + Fm[m]) + G[m];
-      if (store) park[m * (PLANE / 8)] = st.Phip[m] - Phi;
+      if (store) park[m * pstr] = st.Phip[m] - Phi;
       st.Phip[m] = Phi;
     }
   }
@@ -256,7 +261,7 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
       if (j >= p0 + 5) flush((a >> 2) - 1);
       last3 = j;
     }
-    xi_step<1>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4);
+    xi_step<1>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4, reinterpret_cast<double*>(P0), PLANE / 8);  // parked in the Q words of position a-3
     if (ev) {
       // refill the freed slot with the chunk two ahead (if any step will read it); the TMA store issued by flush() must
       // have finished reading the slot first
@@ -272,7 +277,7 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
       const int a1 = a + 1;
       if ((a1 & 3) == 2) wait_chunk((a1 >> 2) + 1);  // position a1+2 opens the next chunk
       P3 = pair_ptr(pb0 + ((j - (p0 - 1)) >> 1) + 3);
-      xi_step<0>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4);
+      xi_step<0>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4, reinterpret_cast<double*>(P0) + 1, PLANE / 8);
       P0 = P1; P1 = P2; P2 = P3;
     }
   }
@@ -287,7 +292,7 @@ k_xi_tma(const __grid_constant__ CUtensorMap tq, const __grid_constant__ CUtenso
 // unit spends ~5 cycles per 32-byte box row (6 B/cycle/SM), which makes the TMA variant TMA-bound (1.41 ms at 256^3);
 // 16-byte LDGSTS with lane -> (line l/2 + 16t, half l%2) writes the same swizzled layout (the XOR done by hand), two
 // lanes cover one sector of a line and a quarter warp writes 128 contiguous bytes.  The flush uses the same lane
-// mapping: LDS.128 of the parked outputs (+ S from its buffer), STG.128 to r.
+// mapping: LDS.128 of the parked outputs, STG.128 to r.
 struct XiLArgs {
   const double* q;    // array origin (ghosts included) of the current q
   const double* kh;   // khat^xi rows
@@ -312,7 +317,8 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
   const int p0 = blockIdx.y * A.S;  // multiple of 4
   const int p1 = min(A.n, p0 + A.S);
   char* const base = smem_raw + ((256u - (smem_u32(smem_raw) & 255u)) & 255u);
-  char* const ring = base + wid * WARP_BYTES;
+  char* const ring = base + wid * XL_WARP_BYTES;
+  char* const obuf = ring + 3 * SLOT;  // side buffer: the first two outputs of a sector group, [5 vars][32 lines][2 positions]
   const int swz = (lane >> 2) & 1;
   const int off0 = lane * 32 + (swz << 4), off1 = lane * 32 + ((swz ^ 1) << 4);
   auto pair_ptr = [&](int pn) -> char* { return ring + ((pn >> 1) % 3) * SLOT + ((pn & 1) ? off1 : off0); };
@@ -341,17 +347,23 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
       for (int cc = 0; cc < 3; ++cc) cp16(slot + (5 + cc) * PLANE + soff[t], L.kh + cc * M + g);
     }
   };
-  // r array positions 4 ch + 2 .. 4 ch + 5 are parked in the Q planes of chunk ch
-  auto flush = [&](int ch, int rlo, int rhi) {  // only r positions in [rlo, rhi) are written
-    const char* const slot = ring + (ch % 3) * SLOT;
-    const int rp = ch * 4 + 2 + 2 * lh - NG;  // first of my two r positions
+  // Outputs leave in SECTOR-ALIGNED groups: group c = r at array indices 4c .. 4c+3 (one full 32-byte sector per line).
+  // Step a produces r at array index x = a-1.  x = 4c, 4c+1 are parked in the side buffer; x = 4c+2, 4c+3 in the Q words of
+  // positions 4c, 4c+1 (pair 0 of chunk c: position x-2 = a-3 is dead for Q).  (Interior position 0 sits at array index
+  // NG = 6, i.e. 16 bytes into a sector: writing the four outputs of a CHUNK, 4c+2 .. 4c+5, would touch two half sectors
+  // per line; measured 1.13 ms against 0.81 ms for this kernel at 256^3.)
+  auto flush = [&](int c, int rlo, int rhi) {  // only r positions in [rlo, rhi) are written
+    const char* const slot = ring + (c % 3) * SLOT;
+    const int rp = c * 4 + 2 * lh - NG;  // first of my two r positions
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
       if (!lok[t]) continue;
-      double* const gr = L.r + goff[t] + ch * 4 + 2;
+      double* const gr = L.r + goff[t] + c * 4;   // goff holds + 2 lh
+      const int ln = lsub + 16 * t;
 #pragma unroll
       for (int m = 0; m < 5; ++m) {
-        double2 v = *reinterpret_cast<const double2*>(slot + m * PLANE + soff[t]);
+        const double2 v = lh == 0 ? *reinterpret_cast<const double2*>(obuf + m * 512 + ln * 16)
+                                  : *reinterpret_cast<const double2*>(slot + m * PLANE + ln * 32 + (((ln >> 2) & 1) << 4));
         if (rp >= rlo && rp + 1 < rhi) *reinterpret_cast<double2*>(gr + m * M) = v;
         else {
           if (rp >= rlo && rp < rhi) gr[m * M] = v.x;
@@ -360,6 +372,7 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
       }
     }
   };
+  double* const opark = reinterpret_cast<double*>(obuf + lane * 16);  // my line's two side-buffer words of variable 0
 
   const int a0 = p0 - 1 + NG;
   const int ch0 = a0 >> 2;
@@ -393,20 +406,24 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
     for (int m = 0; m < 5; ++m) fir_push(st.acc[m], F[m]);
   }
   const double gamma = A.gamma, eps4 = A.eps4;
-  int last3 = -1;
   for (int j = p0 - 1; j <= p1; j += 2) {
     const int a = j + NG;  // odd
-    if ((a & 3) == 3) {
-      // flush the chunk before chunk(a) (its parks are complete), then refill its slot with the chunk two ahead and
-      // fetch S for the chunk being parked now
+    const bool q3 = (a & 3) == 3;
+    if (q3) {
+      // every lane has read the last khat of the chunk before chunk(a): refill its slot with the chunk two ahead
       __syncwarp();
-      if (j >= p0 + 5) flush((a >> 2) - 1, p0, p1);
       const int cn = (a >> 2) + 2;
       if (cn * 4 <= p1 + NG + 2) load_chunk(cn);
       asm volatile("cp.async.commit_group;" ::: "memory");
-      last3 = j;
+    } else if (j >= p0 + 3) {
+      // a = 4c+5: group c is complete (x = 4c+3 was parked by the previous step): write it, then the side buffer is free
+      __syncwarp();
+      flush((a >> 2) - 1, p0, p1);
+      __syncwarp();
     }
-    xi_step<1, SCH>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4);
+    // this step's output x = a-1: side buffer word 0 (a = 1 mod 4) or the Q words of position a-3 (a = 3 mod 4)
+    xi_step<1, SCH>(st, P0, P1, P2, P3, j >= p0, j > p0, gamma, eps4, q3 ? reinterpret_cast<double*>(P0) : opark,
+                    q3 ? PLANE / 8 : 64);
     if (j + 1 <= p1) {
       const int a1 = a + 1;
       if ((a1 & 3) == 2) {  // position a1+2 opens the next chunk
@@ -414,13 +431,16 @@ __global__ void __launch_bounds__(32 * TW, 2) k_xi_ldg(XiLArgs L) {
         __syncwarp();
       }
       P3 = pair_ptr(pb0 + ((j - (p0 - 1)) >> 1) + 3);
-      xi_step<0, SCH>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4);
+      // output x = a: side buffer word 1, or the Q words of position a1-3 = a-2 (second word of pair P0)
+      xi_step<0, SCH>(st, P0, P1, P2, P3, true, j + 1 > p0, gamma, eps4, q3 ? reinterpret_cast<double*>(P0) + 1 : opark + 1,
+                      q3 ? PLANE / 8 : 64);
       P0 = P1; P1 = P2; P2 = P3;
     }
   }
+  // ---- the last group: complete (p1 = 2 mod 4) or its first half only (p1 = 0 mod 4; the rest belongs to the next segment) ----
   asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncwarp();
-  flush((last3 + NG) >> 2, p0, p1);
+  flush((p1 + NG - 1) >> 2, p0, p1);
 }
 
 #undef LD2
