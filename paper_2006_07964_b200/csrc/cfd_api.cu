@@ -9,7 +9,7 @@ static thread_local std::string g_create_err;
 
 static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD_FACE_INTERFACE; }
 
-size_t ws_partials_offset_doubles(const cfd_ctx* c) { return (size_t)WS_ROWS * (size_t)c->sum_M; }
+size_t ws_partials_offset_doubles(const cfd_ctx* c) { return (size_t)WS_ROWS * (size_t)c->sum_M + 8; }  // + 8: past the shifted scratch rows
 int rk_max_partial_blocks() { return 16384; }
 
 extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
@@ -202,7 +202,9 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   c->ws_bytes = workspace_bytes;
   {
     long long off = 0;
-    for (BlockDev& B : c->blk) { B.ws = c->ws + (long long)WS_ROWS * off; off += B.M; }
+    // + 2: the scratch rows are indexed like the fields but shifted by two doubles, so that interior i = 0 (array index NG = 6)
+    // starts a 32-byte sector: the rows are written in interior runs, and half-sector writes cost a read-modify-write
+    for (BlockDev& B : c->blk) { B.ws = c->ws + (long long)WS_ROWS * off + 2; off += B.M; }
   }
   plan_copies(c);
   // ---- small device-side descriptor arrays (a few KB; the only allocations the library makes) ----
