@@ -1,6 +1,7 @@
 """Summarise an Nsight Compute report of the hot kernels into the text files kept under profiles/.
 
     python -m paper_2006_07964_b200.profile_summary REPORT.ncu-rep --workload sweep256 --out profiles/r2 [--command "..."]
+    python -m paper_2006_07964_b200.profile_summary --launches LAUNCHES.csv --out profiles/r2_launches.md [--command "..."]
 
 Reads the report with `ncu -i REPORT --page raw --csv` (no GPU needed) and writes
   <out>_traffic.json    {workload: {kernel class: dram__bytes_read.sum + dram__bytes_write.sum per launch, bytes}}
@@ -16,6 +17,7 @@ import json
 import os
 import re
 import subprocess
+import sys
 
 METRICS = [
     ("gpu__time_duration.sum", "duration"),
@@ -61,7 +63,41 @@ def to_bytes(value: str, unit: str) -> float:
     return float(value.replace(",", "")) * scale
 
 
+def launch_list(csv_path, out_md, command):
+    """Launch list of `ncu --metrics gpu__time_duration.sum --csv --log-file <csv>`: per kernel launches, total and
+    average device time and share (cold caches, serialised launches: compare shares, not absolutes)."""
+    with open(csv_path) as f:
+        lines = [ln for ln in f if not ln.startswith("==")]
+    rows = list(csv.DictReader(lines))
+    agg = {}
+    for r in rows:
+        if r.get("Metric Name") != "gpu__time_duration.sum":
+            continue
+        v = float(r["Metric Value"].replace(",", ""))
+        v *= {"ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3}.get(r.get("Metric Unit", "ns"), 1e-6)
+        k = r["Kernel Name"]
+        a = agg.setdefault(k, [0, 0.0])
+        a[0] += 1
+        a[1] += v
+    tot = sum(v[1] for v in agg.values())
+    out = ["# ncu launch list", "", f"Command: `{command}`", "",
+           "Per-launch times under ncu are cold-cache and serialised: the SHARES are what to compare with bench.py's", 
+           "CUDA-event timing, not the absolutes.", "", "| kernel | launches | total ms | avg ms | share |", "|---|---|---|---|---|"]
+    for k, (n, ms) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+        out.append(f"| `{k[:90]}` | {n} | {ms:.3f} | {ms / n:.4f} | {ms / tot:.3f} |")
+    with open(out_md, "w") as f:
+        f.write("\n".join(out) + "\n")
+    print(f"{len(agg)} kernels, {tot:.2f} ms total -> {out_md}")
+
+
 def main():
+    if len(sys.argv) > 1 and sys.argv[1] == "--launches":
+        ap = argparse.ArgumentParser()
+        ap.add_argument("--launches", required=True, help="csv written by ncu --csv --log-file")
+        ap.add_argument("--out", required=True)
+        ap.add_argument("--command", default="")
+        a = ap.parse_args()
+        return launch_list(a.launches, a.out, a.command)
     ap = argparse.ArgumentParser()
     ap.add_argument("report")
     ap.add_argument("--workload", required=True)
