@@ -41,55 +41,99 @@ static int fail_create(int code, const std::string& msg) {
   return code;
 }
 
-// Host-side plan of the ghost fill (U15): 26 regions per block, each filled through the lowest axis
-// whose face is PERIODIC/INTERFACE; pass = number of out-of-range indices (faces, edges, corners).
+// Host-side plan of the ghost fill (U15).  The fill is defined as three sequential passes (faces, then edges, then corners:
+// the 26 ghost regions of a block, each filled through the lowest out-of-range axis whose face is PERIODIC / INTERFACE,
+// from the neighbour's cells -- which for edges and corners are themselves ghost cells filled by the previous pass).
+// Every such chain ends at cells that no pass writes (interior cells, or ghost cells behind a physical face), and every hop
+// is a signed permutation plus an offset, so the chain is composed HERE into one affine map per region: all regions are
+// filled by ONE launch that reads final sources only (same values, bit for bit, as the three passes).
+struct IdxMap {       // index vector in block `blk` = P x + o for the destination index vector x
+  int blk;
+  int P[3][3];
+  int o[3];
+  double shift[3];    // accumulated coordinate translation (xyz fill)
+};
+
+static bool hop(const cfd_ctx* c, const int ftype[], const int fidx[], IdxMap& m, const int probe[3]) {
+  // where does the probe point sit in the current block?  pick the lowest out-of-range axis behind a connecting face
+  const BlockDev& B = c->blk[m.blk];
+  int y[3];
+  for (int a = 0; a < 3; ++a) y[a] = m.P[a][0] * probe[0] + m.P[a][1] * probe[1] + m.P[a][2] * probe[2] + m.o[a];
+  int an = -1, s = 0;
+  for (int a = 0; a < 3 && an < 0; ++a) {
+    if (y[a] >= 0 && y[a] < B.n[a]) continue;
+    const int fc = 2 * a + (y[a] < 0 ? 0 : 1);
+    if (is_connect(ftype[m.blk * 6 + fc])) { an = a; s = fc % 2; }
+  }
+  if (an < 0) return false;
+  const cfd_face& F = c->faces[fidx[m.blk * 6 + 2 * an + s]];
+  const BlockDev& N = c->blk[F.nbr_block];
+  const int sp = F.nbr_face % 2;
+  IdxMap r;
+  r.blk = F.nbr_block;
+  for (int a = 0; a < 3; ++a) {
+    const int ap = F.perm[a];
+    int sgn, off;
+    if (a == an) {
+      if (s == 0 && sp == 1) { sgn = 1; off = N.n[ap]; }
+      else if (s == 0 && sp == 0) { sgn = -1; off = -1; }
+      else if (s == 1 && sp == 0) { sgn = 1; off = -B.n[a]; }
+      else { sgn = -1; off = N.n[ap] + B.n[a] - 1; }
+    } else {
+      sgn = F.sign[a] > 0 ? 1 : -1;
+      off = F.sign[a] > 0 ? 0 : B.n[a] - 1;
+    }
+    // neighbour index along ap = sgn * (my index along a) + off, my index = row a of (P x + o)
+    for (int t = 0; t < 3; ++t) r.P[ap][t] = sgn * m.P[a][t];
+    r.o[ap] = sgn * m.o[a] + off;
+  }
+  for (int t = 0; t < 3; ++t) r.shift[t] = m.shift[t] + F.shift[t];
+  m = r;
+  return true;
+}
+
 static void plan_copies(cfd_ctx* c) {
-  for (size_t b = 0; b < c->blk.size(); ++b) {
+  const size_t nb = c->blk.size();
+  std::vector<int> ftype(nb * 6, 0), fidx(nb * 6, -1);
+  for (size_t t = 0; t < c->faces.size(); ++t) {
+    ftype[(size_t)c->faces[t].block * 6 + c->faces[t].face] = c->faces[t].type;
+    fidx[(size_t)c->faces[t].block * 6 + c->faces[t].face] = (int)t;
+  }
+  for (size_t b = 0; b < nb; ++b) {
     const BlockDev& B = c->blk[b];
-    int ftype[6], fidx[6];
-    for (int s = 0; s < 6; ++s) { ftype[s] = 0; fidx[s] = -1; }
-    for (size_t t = 0; t < c->faces.size(); ++t)
-      if (c->faces[t].block == (int)b) { ftype[c->faces[t].face] = c->faces[t].type; fidx[c->faces[t].face] = (int)t; }
     for (int code = 0; code < 27; ++code) {
       int side[3] = {code % 3, (code / 3) % 3, code / 9};  // 0 below, 1 inside, 2 above
-      int nout = 0, fsel = -1;
-      for (int a = 0; a < 3; ++a) {
-        if (side[a] == 1) continue;
-        ++nout;
-        int fc = 2 * a + (side[a] == 2 ? 1 : 0);
-        if (fsel < 0 && is_connect(ftype[fc])) fsel = fc;
-      }
-      if (nout == 0 || fsel < 0) continue;
-      const cfd_face& F = c->faces[fidx[fsel]];
-      const BlockDev& N = c->blk[F.nbr_block];
+      if (code == 13) continue;
       CopyTask T;
       T.dst_block = (int)b;
-      T.src_block = F.nbr_block;
-      T.pass = nout;
+      int probe[3];
       for (int a = 0; a < 3; ++a) {
         T.lo[a] = side[a] == 0 ? -NG : (side[a] == 1 ? 0 : B.n[a]);
         T.ext[a] = side[a] == 1 ? B.n[a] : NG;
-        T.shift[a] = F.shift[a];
+        probe[a] = T.lo[a];
       }
-      const int an = F.face / 2, s = F.face % 2, sp = F.nbr_face % 2;
-      long long base = 0;
+      IdxMap m;
+      m.blk = (int)b;
       for (int a = 0; a < 3; ++a) {
-        const int ap = F.perm[a];
-        int sgn, off;
-        if (a == an) {
-          if (s == 0 && sp == 1) { sgn = 1; off = N.n[ap]; }
-          else if (s == 0 && sp == 0) { sgn = -1; off = -1; }
-          else if (s == 1 && sp == 0) { sgn = 1; off = -B.n[a]; }
-          else { sgn = -1; off = N.n[ap] + B.n[a] - 1; }
-        } else {
-          sgn = F.sign[a] > 0 ? 1 : -1;
-          off = F.sign[a] > 0 ? 0 : B.n[a] - 1;
-        }
-        T.sstride[a] = sgn * N.s[ap];
-        base += (long long)(off + NG) * N.s[ap];
+        for (int t = 0; t < 3; ++t) m.P[a][t] = a == t ? 1 : 0;
+        m.o[a] = 0;
+        m.shift[a] = 0.0;
+      }
+      int hops = 0;
+      while (hops < 3 && hop(c, ftype.data(), fidx.data(), m, probe)) ++hops;
+      if (hops == 0) continue;  // no connecting face behind this region: the physical boundary conditions own it
+      const BlockDev& S = c->blk[m.blk];
+      T.src_block = m.blk;
+      long long base = 0;
+      for (int t = 0; t < 3; ++t) T.sstride[t] = 0;
+      for (int a = 0; a < 3; ++a) {
+        for (int t = 0; t < 3; ++t) T.sstride[t] += (long long)m.P[a][t] * S.s[a];
+        base += (long long)(m.o[a] + NG) * S.s[a];
+        T.shift[a] = m.shift[a];
       }
       T.sbase = base;
-      c->tasks[nout].push_back(T);
+      T.pass = 1;
+      c->tasks[1].push_back(T);
     }
   }
 }
