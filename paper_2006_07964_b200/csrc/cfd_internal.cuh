@@ -74,6 +74,7 @@ struct cfd_ctx {
   static constexpr int NSIDE = 4;     // side streams: the blocks of a multi-block case run their per-block kernels concurrently
   cudaStream_t side[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
   cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
+  int conc = 1;                       // blocks whose kernel chains run concurrently (side streams): the sweeps size their segments for conc x their own CTAs
   long long launches = 0;
   int xi_mode = 0;                    // xi kernel (cfd_set_sweep_plan): 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
   std::string err;

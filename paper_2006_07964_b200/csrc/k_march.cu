@@ -525,7 +525,7 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
   A.nl = B.n[la]; A.nt = B.n[ta]; A.n = B.n[dir];
   const long long lanes = (long long)A.nl * A.nt;
   const long long ctas_per_seg = (lanes + MT - 1) / MT;
-  int nseg = pick_segments(ctas_per_seg, A.n, 1);
+  int nseg = pick_segments(ctas_per_seg * c->conc, A.n, 1);
   if (rk && rk->stage == 1) {
     while (nseg > 1 && ctas_per_seg * nseg > rk->max_ctas) --nseg;
     if (ctas_per_seg * nseg > rk->max_ctas) { c->err = "fused RK stage: block too large for the residual partials"; return CFD_E_WORKSPACE; }
@@ -575,7 +575,7 @@ int launch_march_xi(cfd_ctx* c, const BlockDev& B) {
   A.nlb = (A.nl + 31) / 32;
   A.ph = (4 - (NG & 3)) & 3;
   const long long units = (long long)A.nlb * A.nt;
-  const int nseg = pick_segments((units + XWARPS - 1) / XWARPS, A.n, 1);
+  const int nseg = pick_segments((units + XWARPS - 1) / XWARPS * c->conc, A.n, 1);
   A.S = (A.n + nseg - 1) / nseg;
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;

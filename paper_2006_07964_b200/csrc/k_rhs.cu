@@ -54,6 +54,8 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
     for (int t = 0; t < cfd_ctx::NSIDE; ++t) CUDA_TRY(c, cudaStreamWaitEvent(c->side[t], c->ev_fork, 0));
   }
   int bi = 0, rc = 0;
+  // the sweeps size their segments for the CTAs of all concurrently running blocks (C4: 3.31 -> 3.48 Gpts/s)
+  c->conc = fork ? (int)(c->blk.size() < (size_t)cfd_ctx::NSIDE ? c->blk.size() : (size_t)cfd_ctx::NSIDE) : 1;
   for (const BlockDev& B : c->blk) {
     if (fork) c->stream = c->side[bi++ % cfd_ctx::NSIDE];
     if (c->pd.viscous) {

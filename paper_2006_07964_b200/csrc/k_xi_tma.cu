@@ -533,7 +533,7 @@ int launch_xi_tma(cfd_ctx* c, int b, bool tma) {
   A.nlb = (A.nl + 31) / 32;
   const long long units = (long long)A.nlb * A.nt;
   const long long ctas = (units + TW - 1) / TW;
-  const int nseg = pick_segments(ctas, A.n, 4);
+  const int nseg = pick_segments(ctas * c->conc, A.n, 4);
   A.S = (((A.n + nseg - 1) / nseg) + 3) & ~3;
   A.gamma = c->pd.gamma;
   A.eps4 = 4.0 * c->pd.eps;
