@@ -113,7 +113,8 @@ __device__ __forceinline__ PrimD prims_of(const double Q[5], double gamma) {
 
 __global__ void __launch_bounds__(128) k_bc_q(BlockDev B, ParamsDev P, int face, int type) {
   const int an = face / 2, s = face % 2;
-  const int t1 = (an + 1) % 3, t2 = (an + 2) % 3;
+  // tangential axes, the lower one fastest across threads (i when the face is not a xi face: coalesced)
+  const int t1 = an == 0 ? 1 : 0, t2 = an == 2 ? 1 : 2;
   const int e1 = B.n[t1] + 6, e2 = B.n[t2] + 6;
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= e1 * e2) return;
