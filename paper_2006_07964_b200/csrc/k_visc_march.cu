@@ -1,28 +1,34 @@
-// S3 up to the point fluxes as ONE k-marching kernel (replaces k_phi + k_visc_flux<true> on the default plan).
-// sm_100a, fp64.  P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.  Shares no code with oracle/.
+// S3 up to the point fluxes as ONE k-marching kernel.   sm_100a, fp64.
+// P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.  Shares no code with oracle/.
 //
-// k_visc_flux reads 72 neighbour values of phi per point through L1 (latency-bound: DRAM 44 %, LSU wavefronts 62 %) and
-// needs phi stored by a separate pass.  Here a CTA owns a tile of (i, j) columns and marches along k:
+// A CTA owns a tile of (i, j) columns and marches along k:
 //   * phi = (u, v, w, T) is computed from Q on the fly and never stored;
-//   * the zeta stencil lives in REGISTERS: each thread keeps phi of its own column at k-3 .. k+3 (28 doubles);
+//   * the zeta stencil lives in REGISTERS: each thread keeps phi of its own column at k-3 .. k+3 (28 doubles).  The k loop
+//     is unrolled SEVEN times with the register names rotating, so the pipeline is never shifted (the shifts were 36 of the
+//     ~735 instructions of a step);
 //   * the (i, j) plane of phi at k (tile + halo of 3 in j, 6 in i) lives in SHARED memory, double buffered: the xi and
 //     eta stencils read it with LDS;
 //   * Q of plane k+4 and the halo cells of plane k+1 arrive by cp.async in thread-private shared-memory slots one step
 //     ahead (no registers held across a step); the ten metric values of plane k+1 are loaded at the end of step k, when few
-//     registers are live (staging them through shared memory cost more shared-memory instructions than it hid latency);
-//   * the xi rows of the flux go to shared memory and come back as S = d(Fv^xi)/d(xi), as in k_visc_flux<true>.
+//     registers are live;
+//   * the xi rows of the flux go to shared memory and come back as S = d(Fv^xi)/d(xi).
+// Addressing: one 32-bit element offset per thread (its column at the current plane) on top of per-row base pointers that
+// arrive as kernel parameters: one IMAD.WIDE per global access.  (With 64-bit offsets recomputed from the block
+// descriptor the compiler, capped at 128 registers, rematerialised ~200 integer instructions per step.)  Columns that
+// stick out of the array are clamped onto its last column instead of predicated: they compute and never store.
 // Output (workspace rows): W[0..3] = S on interior points; W[4..7] = Fv^eta rows 2..5 on (i, k) interior, j in [-3, nj+3);
-// W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).  Same arithmetic per point as k_phi + k_visc_flux.
+// W[8..11] = Fv^zeta rows 2..5 on (i, j) interior, k in [-3, nk+3).
 #include "cfd_internal.cuh"
 #include "fastmath.cuh"
 #include "stencil.cuh"
 #include <cmath>
+#include <type_traits>
 
 namespace {
 
 // Tile geometry: VX x VY threads own the columns i0-3 .. i0+VX-4 of the rows j0 .. j0+VY-1; VX-6 of them are output columns.
 // The plane row pitch PC is congruent to VX modulo 16 doubles, so that consecutive threads (also across a row change
-// inside a warp when VX is not a multiple of 32) hit consecutive banks.  Every thread stages HPT halo cells of the plane.
+// inside a warp when VX is not a multiple of 32) hit consecutive banks.  Every thread stages at most one halo cell.
 template <int VX_, int VY_>
 struct VG {
   static constexpr int VX = VX_, VY = VY_;
@@ -30,15 +36,30 @@ struct VG {
   static constexpr int PR = VY + 6;           // plane rows j0-3 .. j0+VY+2
   static constexpr int NHALO = 2 * 3 * VX + 2 * 3 * VY;
   static constexpr int NT = VX * VY;
-  static constexpr int HPT = (NHALO + NT - 1) / NT;   // halo cells staged per thread
   static constexpr int MINB = NT <= 256 ? 2 : 1;      // CTAs per SM (128 registers per thread either way)
-  static_assert(NT <= 512, "k_visc_march: tile geometry");
-  // shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [2][4][VY][VX] | Q stage [5][NT] | halo stage [5][HPT NT]
-  static constexpr int SM_PHI = 2 * 4 * PR * PC, SM_WX = 2 * 4 * NT, SM_Q = 5 * NT, SM_H = 5 * HPT * NT;
+  static_assert(NT <= 512 && NHALO <= NT, "k_visc_march: tile geometry");
+  // shared memory (doubles): phi planes [2][4][PR][PC] | xi rows [2][4][VY][VX] | Q stage [5][NT] | halo stage [5][NT]
+  static constexpr int SM_PLANE = 4 * PR * PC, SM_WXB = 4 * NT;
+  static constexpr int SM_PHI = 2 * SM_PLANE, SM_WX = 2 * SM_WXB, SM_Q = 5 * NT, SM_H = 5 * NT;
   static constexpr int SMEM = (SM_PHI + SM_WX + SM_Q + SM_H) * 8;
 };
 
-// phi = (u, v, w, T = gamma p / rho) from the conservative state: the arithmetic of k_phi
+// Row base pointers (array origin) and sizes: everything the kernel reads from its parameters
+struct ViscArgs {
+  const double* q[5];
+  const double* kh[9];
+  const double* jac;
+  double* w[12];
+  int n[3], m[3];
+  unsigned s1, s2;    // row and plane pitch in doubles
+  int TI, KS;
+  double gamma, mu, kappa, suth;
+};
+
+// thread roles, packed in one register
+constexpr unsigned F_XI = 1u, F_ETA = 2u, F_ZETA = 4u, F_S = 8u, F_ANY = 16u, F_HALO = 32u;
+
+// phi = (u, v, w, T = gamma p / rho) from the conservative state
 __device__ __forceinline__ void phi_of(double r, double m1, double m2, double m3, double e, double gamma, double f[4]) {
   const double ir = frcp(r);
   const double u = m1 * ir, v = m2 * ir, w = m3 * ir;
@@ -47,149 +68,145 @@ __device__ __forceinline__ void phi_of(double r, double m1, double m2, double m3
 }
 
 template <class G>
-__global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, ParamsDev P, double* __restrict__ W, int TI, int KS) {
-  constexpr int VX = G::VX, VY = G::VY, PC = G::PC, PR = G::PR, NHALO = G::NHALO, NT = G::NT, HPT = G::HPT;
-  constexpr int SM_PHI = G::SM_PHI, SM_WX = G::SM_WX, SM_Q = G::SM_Q;
+__global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(const __grid_constant__ ViscArgs A) {
+  constexpr int VX = G::VX, VY = G::VY, PC = G::PC, PR = G::PR, NHALO = G::NHALO, NT = G::NT;
   extern __shared__ double vsm[];
-  double* const sphi = vsm;               // [2][4][PR][PC]
-  double* const swx = sphi + SM_PHI;      // [2][4][VY][VX]
-  double* const sq = swx + SM_WX;         // [5][NT]
-  double* const sh = sq + SM_Q;           // [5][HPT NT]
+  double* const sphi = vsm;                 // [2][4][PR][PC]
+  double* const swx = sphi + G::SM_PHI;     // [2][4][VY][VX]
+  double* const sq = swx + G::SM_WX;        // [5][NT]
+  double* const sh = sq + G::SM_Q;          // [5][NT]
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * VX + tx;
-  const int i0 = blockIdx.x * TI, j0 = -3 + (int)blockIdx.y * VY;
-  const int kb = -3 + (int)blockIdx.z * KS, ke = min(kb + KS, B.n[2] + 3);
+  const int i0 = blockIdx.x * A.TI, j0 = -3 + (int)blockIdx.y * VY;
+  const int kb = -3 + (int)blockIdx.z * A.KS, ke = min(kb + A.KS, A.n[2] + 3);
   const int i = i0 - 3 + tx, j = j0 + ty;
-  const long long M = B.M, s1 = B.s[1], s2 = B.s[2];
-  const double gamma = P.gamma;
-  // my column: inside the array?  (plane filler)   which results are wanted from it?
-  const bool col_in = (i + NG < B.m[0]) && (j + NG < B.m[1]);
-  const bool oi = i < 0 || i >= B.n[0], oj = j < 0 || j >= B.n[1];
-  const bool own = tx >= 3 && tx < TI + 3 && i < B.n[0];                       // point-wise outputs are mine
-  const bool want_xi = tx < TI + 6 && i < B.n[0] + 3 && !oj;                    // xi rows (k interior)
-  const bool want_eta = own && j < B.n[1] + 3;                                  // eta rows (k interior)
-  const bool want_zeta = own && !oj;                                            // zeta rows (all k of the march)
-  const bool any = col_in && (want_xi || want_eta || want_zeta) && !(oi && oj);
-  const long long pcol = (long long)(j + NG) * s1 + (i + NG);                  // array offset of (i, j, k = -NG)
-  // my halo cells of the plane (if any): top band, bottom band, left columns, right columns
-  int hpl[HPT];           // offset of the cell inside one field of the plane (hr * PC + hc)
-  bool halo_in[HPT];
-  long long phal[HPT];
-#pragma unroll
-  for (int h = 0; h < HPT; ++h) {
-    const int t = tid + h * NT;
-    int hc = -1, hr = -1;  // plane column / row
-    if (t < 3 * VX) { hr = t / VX; hc = 3 + t % VX; }
-    else if (t < 6 * VX) { hr = VY + 3 + (t - 3 * VX) / VX; hc = 3 + t % VX; }
-    else if (t < 6 * VX + 3 * VY) { hr = 3 + (t - 6 * VX) / 3; hc = (t - 6 * VX) % 3; }
-    else if (t < NHALO) { hr = 3 + (t - 6 * VX - 3 * VY) / 3; hc = VX + 3 + (t - 6 * VX - 3 * VY) % 3; }
+  const unsigned s2 = A.s2;
+  const double gamma = A.gamma;
+  unsigned flags = 0;
+  unsigned p;      // element offset of my column at the current plane
+  int dh = 0;      // my halo cell's column minus my own (elements)
+  int hpl = 0;     // my halo cell inside one field of the plane
+  {
+    const bool col_in = (i + NG < A.m[0]) && (j + NG < A.m[1]);
+    const bool oi = i < 0 || i >= A.n[0], oj = j < 0 || j >= A.n[1];
+    const bool own = tx >= 3 && tx < A.TI + 3 && i < A.n[0];                     // point-wise outputs are mine
+    const bool want_xi = tx < A.TI + 6 && i < A.n[0] + 3 && !oj;                  // xi rows (k interior)
+    const bool want_eta = own && j < A.n[1] + 3;                                  // eta rows (k interior)
+    const bool want_zeta = own && !oj;                                            // zeta rows (all k of the march)
+    if (col_in && want_xi) flags |= F_XI;
+    if (col_in && want_eta) flags |= F_ETA;
+    if (col_in && want_zeta) flags |= F_ZETA | F_S;
+    if (col_in && (want_xi || want_eta || want_zeta) && !(oi && oj)) flags |= F_ANY;
+    const int ic = min(i, A.m[0] - NG - 1), jc = min(j, A.m[1] - NG - 1);         // clamped onto the array
+    const unsigned pc = (unsigned)(jc + NG) * A.s1 + (unsigned)(ic + NG);
+    p = pc + (unsigned)(kb + NG) * s2;
+    // my halo cell of the plane (if any): top band, bottom band, left columns, right columns
+    int hc = -1, hr = 0;
+    if (tid < 3 * VX) { hr = tid / VX; hc = 3 + tid % VX; }
+    else if (tid < 6 * VX) { hr = VY + 3 + (tid - 3 * VX) / VX; hc = 3 + tid % VX; }
+    else if (tid < 6 * VX + 3 * VY) { hr = 3 + (tid - 6 * VX) / 3; hc = (tid - 6 * VX) % 3; }
+    else if (tid < NHALO) { hr = 3 + (tid - 6 * VX - 3 * VY) / 3; hc = VX + 3 + (tid - 6 * VX - 3 * VY) % 3; }
     const int hi = i0 - 6 + hc, hj = j0 - 3 + hr;
-    halo_in[h] = hc >= 0 && hi + NG >= 0 && hi + NG < B.m[0] && hj + NG >= 0 && hj + NG < B.m[1];
-    phal[h] = (long long)(hj + NG) * s1 + (hi + NG);
-    hpl[h] = hr * PC + hc;
-  }
-
-  auto stage = [&](int k) {  // cp.async for the step of plane k: Q(k+3) of my column, my halo cell at k, metrics at k
-    if (col_in && k + 3 + NG < B.m[2]) {
-      const long long o = pcol + (long long)(k + 3 + NG) * s2;
-#pragma unroll
-      for (int m = 0; m < 5; ++m) cp8(sq + m * NT + tid, B.q + m * M + o);
+    if (hc >= 0 && hi + NG >= 0 && hi + NG < A.m[0] && hj + NG >= 0 && hj + NG < A.m[1]) {
+      flags |= F_HALO;
+      dh = (int)((unsigned)(hj + NG) * A.s1 + (unsigned)(hi + NG)) - (int)pc;
+      hpl = hr * PC + hc;
     }
+  }
+  double* const myq = sq + tid;
+  double* const myh = sh + tid;
+  double* const mypl = sphi + (ty + 3) * PC + tx + 3;   // my own cell in field 0 of plane buffer 0
+  double* const mywx = swx + ty * VX + tx;              // my xi-row cell, row 0 of buffer 0
+
+  // cp.async for the step of the plane at offset pp: Q three planes further of my column, my halo cell of that plane
+  auto stage = [&](unsigned pp) {
+    const unsigned o = pp + 3u * s2;
 #pragma unroll
-    for (int h = 0; h < HPT; ++h) {
-      if (halo_in[h]) {
-        const long long o = phal[h] + (long long)(k + NG) * s2;
+    for (int m = 0; m < 5; ++m) cp8(myq + m * NT, A.q[m] + o);
+    if (flags & F_HALO) {
+      const unsigned oh = pp + (unsigned)dh;
 #pragma unroll
-        for (int m = 0; m < 5; ++m) cp8(sh + (m * HPT + h) * NT + tid, B.q + m * M + o);
-      }
+      for (int m = 0; m < 5; ++m) cp8(myh + m * NT, A.q[m] + oh);
     }
     cp_commit();
   };
-
-  // ---- prologue: phi of my column at kb-3 .. kb+2 ----
-  double ph[7][4];
-#pragma unroll
-  for (int t = 0; t < 7; ++t)
-#pragma unroll
-    for (int f = 0; f < 4; ++f) ph[t][f] = 0.0;
-  if (col_in) {
-#pragma unroll
-    for (int t = 0; t < 6; ++t) {
-      const long long o = pcol + (long long)(kb - 3 + t + NG) * s2;
-      phi_of(B.q[o], B.q[M + o], B.q[2 * M + o], B.q[3 * M + o], B.q[4 * M + o], gamma, ph[t]);
-    }
-  }
-  stage(kb);
-  // the ten metric values of plane k are loaded at the END of step k-1 (after its flux arithmetic, when few registers are
-  // live) and used in the second half of step k: half a step of distance covers the DRAM latency of these streaming loads
   double kh[3][3], J = 0.0;
 #pragma unroll
   for (int d = 0; d < 3; ++d)
 #pragma unroll
     for (int c = 0; c < 3; ++c) kh[d][c] = 0.0;
-  auto load_metrics = [&](int k) {
-    if (any) {
-      const long long o = pcol + (long long)(k + NG) * s2;
+  auto load_metrics = [&](unsigned pp) {
+    if (flags & F_ANY) {
 #pragma unroll
       for (int d = 0; d < 3; ++d)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) kh[d][c] = __ldg(B.khat + (d * 3 + c) * M + o);
-      J = __ldg(B.jac + o);
+        for (int c = 0; c < 3; ++c) kh[d][c] = __ldg(A.kh[d * 3 + c] + pp);
+      J = __ldg(A.jac + pp);
     }
   };
-  load_metrics(kb);
-  const double mu0 = P.mu, kap0 = P.kappa, suth = P.suth;
-  auto s_of_plane = [&](int kk) {
-    if (own && !oj && col_in && kk >= 0 && kk < B.n[2]) {
-      const long long p = pcol + (long long)(kk + NG) * s2;
-      const double* const sx = swx + (kk & 1) * (4 * NT);
+
+  // ---- prologue: phi of my column at kb-3 .. kb+2 (pipeline slots 0 .. 5 of rotation 0) ----
+  double ph[7][4];
 #pragma unroll
-      for (int m = 0; m < 4; ++m) {
-        const double* a = sx + (m * VY + ty) * VX + tx;
-        W[(long long)m * M + p] = d6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
-      }
-    }
+  for (int t = 0; t < 6; ++t) {
+    const unsigned o = p + (unsigned)(t - 3) * s2;
+    phi_of(A.q[0][o], A.q[1][o], A.q[2][o], A.q[3][o], A.q[4][o], gamma, ph[t]);
+  }
+#pragma unroll
+  for (int f = 0; f < 4; ++f) ph[6][f] = 0.0;
+  stage(p);
+  load_metrics(p);
+  const double mu0 = A.mu, kap0 = A.kappa, suth = A.suth;
+  unsigned par = 0;   // plane / xi-row buffer of the current step
+
+  // S = d(Fv^xi)/d(xi) of the plane whose xi rows sit in buffer b, stored at offset pp
+  auto s_of_plane = [&](unsigned b, unsigned pp) {
+    const double* a = mywx + b * G::SM_WXB;
+#pragma unroll
+    for (int m = 0; m < 4; ++m, a += NT) A.w[m][pp] = d6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
   };
-  for (int k = kb; k < ke; ++k) {
+
+  // One plane step; R = rotation of the register pipeline: plane k-3+t lives in ph[(t + R) % 7].
+  // prev_in / cur_in: plane k-1 / k is an interior plane (uniform).
+  auto step = [&](auto Rc, bool prev_in, bool cur_in, bool more) {
+    constexpr int R = decltype(Rc)::value;
+    double(&c0)[4] = ph[(0 + R) % 7]; double(&c1)[4] = ph[(1 + R) % 7]; double(&c2)[4] = ph[(2 + R) % 7];
+    double(&c3)[4] = ph[(3 + R) % 7]; double(&c4)[4] = ph[(4 + R) % 7]; double(&c5)[4] = ph[(5 + R) % 7];
+    double(&c6)[4] = ph[(6 + R) % 7];
     cp_wait<0>();
-    const bool ok = k < 0 || k >= B.n[2];
-    double* const pl = sphi + (k & 1) * (4 * PR * PC);
+    double* const pl = mypl + par * G::SM_PLANE;
     // ---- newest plane of my column into the register pipeline; plane k (my own phi and my halo cell) into shared memory ----
-    if (col_in && k + 3 + NG < B.m[2])
-      phi_of(sq[tid], sq[NT + tid], sq[2 * NT + tid], sq[3 * NT + tid], sq[4 * NT + tid], gamma, ph[6]);
+    phi_of(myq[0], myq[NT], myq[2 * NT], myq[3 * NT], myq[4 * NT], gamma, c6);
 #pragma unroll
-    for (int f = 0; f < 4; ++f) pl[(f * PR + ty + 3) * PC + tx + 3] = ph[3][f];
+    for (int f = 0; f < 4; ++f) pl[f * PR * PC] = c3[f];
+    if (flags & F_HALO) {
+      double hf[4];
+      phi_of(myh[0], myh[NT], myh[2 * NT], myh[3 * NT], myh[4 * NT], gamma, hf);
+      double* const hp = sphi + par * G::SM_PLANE + hpl;
 #pragma unroll
-    for (int h = 0; h < HPT; ++h) {
-      if (halo_in[h]) {
-        double hf[4];
-        const double* a = sh + h * NT + tid;
-        phi_of(a[0], a[HPT * NT], a[2 * HPT * NT], a[3 * HPT * NT], a[4 * HPT * NT], gamma, hf);
-#pragma unroll
-        for (int f = 0; f < 4; ++f) pl[f * PR * PC + hpl[h]] = hf[f];
-      }
+      for (int f = 0; f < 4; ++f) hp[f * PR * PC] = hf[f];
     }
-    if (k + 1 < ke) stage(k + 1);
+    if (more) stage(p + s2);
     __syncthreads();
-    // S = d(Fv^xi)/d(xi) of the PREVIOUS plane: its xi rows were written before this barrier (one barrier per step)
-    if (k > kb) s_of_plane(k - 1);
-    const bool do_xi = want_xi && !ok && col_in;
-    const bool do_eta = want_eta && !ok && !oi && col_in;
-    const bool do_zeta = want_zeta && !oi && col_in;
+    // S of the PREVIOUS plane: its xi rows were written before this barrier (one barrier per step)
+    if (prev_in && (flags & F_S)) s_of_plane(par ^ 1u, p - s2);
+    const bool do_xi = cur_in && (flags & F_XI);
+    const bool do_eta = cur_in && (flags & F_ETA);
+    const bool do_zeta = (flags & F_ZETA) != 0;
     if (do_xi || do_eta || do_zeta) {
       double g[3][4];
 #pragma unroll
       for (int f = 0; f < 4; ++f) {
-        const double* a = pl + (f * PR + ty + 3) * PC + tx + 3;
+        const double* a = pl + f * PR * PC;
         const double dx = d6c(a[-3], a[-2], a[-1], a[1], a[2], a[3]);
         const double dy = d6c(a[-3 * PC], a[-2 * PC], a[-PC], a[PC], a[2 * PC], a[3 * PC]);
-        const double dz = d6c(ph[0][f], ph[1][f], ph[2][f], ph[4][f], ph[5][f], ph[6][f]);
+        const double dz = d6c(c0[f], c1[f], c2[f], c4[f], c5[f], c6[f]);
 #pragma unroll
         for (int c = 0; c < 3; ++c) g[c][f] = J * ((kh[0][c] * dx + kh[1][c] * dy) + kh[2][c] * dz);
       }
-      const double u = ph[3][0], v = ph[3][1], w = ph[3][2];
+      const double u = c3[0], v = c3[1], w = c3[2];
       double mu = mu0, kap = kap0;
       if (suth > 0.0) {  // mu(T) by Sutherland's law (U11): uniform branch
-        const double f = sutherland_factor(ph[3][3], suth);
+        const double f = sutherland_factor(c3[3], suth);
         mu *= f; kap *= f;
       }
       const double lam = -(2.0 / 3.0) * mu;
@@ -203,7 +220,6 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
       const double bx = u * txx + v * txy + w * txz + kap * g[0][3];
       const double by = u * txy + v * tyy + w * tyz + kap * g[1][3];
       const double bz = u * txz + v * tyz + w * tzz + kap * g[2][3];
-      const long long p = pcol + (long long)(k + NG) * s2;
 #pragma unroll
       for (int d = 0; d < 3; ++d) {
         if ((d == 0 && !do_xi) || (d == 1 && !do_eta) || (d == 2 && !do_zeta)) continue;
@@ -213,23 +229,36 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(BlockDev B, Param
         const double w2 = a * txz + b * tyz + c * tzz;
         const double w3 = a * bx + b * by + c * bz;
         if (d == 0) {
-          double* const sx = swx + (k & 1) * (4 * NT);
-          sx[(0 * VY + ty) * VX + tx] = w0; sx[(1 * VY + ty) * VX + tx] = w1;
-          sx[(2 * VY + ty) * VX + tx] = w2; sx[(3 * VY + ty) * VX + tx] = w3;
+          double* const sx = mywx + par * G::SM_WXB;
+          sx[0] = w0; sx[NT] = w1; sx[2 * NT] = w2; sx[3 * NT] = w3;
         } else {
-          W[(d * 4 + 0) * M + p] = w0; W[(d * 4 + 1) * M + p] = w1;
-          W[(d * 4 + 2) * M + p] = w2; W[(d * 4 + 3) * M + p] = w3;
+          A.w[d * 4 + 0][p] = w0; A.w[d * 4 + 1][p] = w1;
+          A.w[d * 4 + 2][p] = w2; A.w[d * 4 + 3][p] = w3;
         }
       }
     }
-    if (k + 1 < ke) load_metrics(k + 1);
-#pragma unroll
-    for (int t = 0; t < 6; ++t)
-#pragma unroll
-      for (int f = 0; f < 4; ++f) ph[t][f] = ph[t + 1][f];
+    if (more) load_metrics(p + s2);
+    p += s2;
+    par ^= 1u;
+  };
+
+  const int n2 = A.n[2];
+  int k = kb;
+#define VSTEP(R)                                                                                                    \
+  step(std::integral_constant<int, R>{}, (unsigned)(k - 1) < (unsigned)n2 && k > kb, (unsigned)k < (unsigned)n2, k + 1 < ke); \
+  ++k;
+  while (true) {
+    VSTEP(0) if (k >= ke) break;
+    VSTEP(1) if (k >= ke) break;
+    VSTEP(2) if (k >= ke) break;
+    VSTEP(3) if (k >= ke) break;
+    VSTEP(4) if (k >= ke) break;
+    VSTEP(5) if (k >= ke) break;
+    VSTEP(6) if (k >= ke) break;
   }
+#undef VSTEP
   __syncthreads();
-  s_of_plane(ke - 1);
+  if ((unsigned)(ke - 1) < (unsigned)n2 && (flags & F_S)) s_of_plane(par ^ 1u, p - s2);
 }
 
 using G0 = VG<64, 8>;
@@ -246,6 +275,7 @@ int visc_march_init() {
 // per-plane barrier, not by the tile's halo overhead -- so only this one is instantiated.
 int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
   using G = G0;
+  if (B.M + 2 >= (1LL << 32)) { c->err = "k_visc_march: block too large for 32-bit element offsets"; return CFD_E_ARG; }
   const int TImax = G::VX - 6;
   const int ntile = (B.n[0] + TImax - 1) / TImax;
   const int TI = (B.n[0] + ntile - 1) / ntile;
@@ -263,8 +293,17 @@ int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
     if (eff > best + 1e-9) { best = eff; nseg = ns; }
   }
   const int KS = (nk + nseg - 1) / nseg;
+  ViscArgs A;
+  for (int m = 0; m < 5; ++m) A.q[m] = B.q + (long long)m * B.M;
+  for (int m = 0; m < 9; ++m) A.kh[m] = B.khat + (long long)m * B.M;
+  A.jac = B.jac;
+  for (int m = 0; m < 12; ++m) A.w[m] = B.ws + (long long)m * B.M;
+  for (int a = 0; a < 3; ++a) { A.n[a] = B.n[a]; A.m[a] = B.m[a]; }
+  A.s1 = (unsigned)B.s[1]; A.s2 = (unsigned)B.s[2];
+  A.TI = TI; A.KS = KS;
+  A.gamma = c->pd.gamma; A.mu = c->pd.mu; A.kappa = c->pd.kappa; A.suth = c->pd.suth;
   dim3 grid(ntile, rows, (nk + KS - 1) / KS);
-  k_visc_march<G><<<grid, dim3(G::VX, G::VY), G::SMEM, c->stream>>>(B, c->pd, B.ws, TI, KS);
+  k_visc_march<G><<<grid, dim3(G::VX, G::VY), G::SMEM, c->stream>>>(A);
   c->launches++;
   return 0;
 }
