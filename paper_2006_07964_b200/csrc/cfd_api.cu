@@ -133,6 +133,7 @@ static void plan_copies(cfd_ctx* c) {
       }
       T.sbase = base;
       T.pass = 1;
+      T.cta_begin = c->tasks[1].empty() ? 0 : c->tasks[1].back().cta_begin + fill_ctas_of(c->tasks[1].back());
       c->tasks[1].push_back(T);
     }
   }

@@ -44,7 +44,8 @@ struct CopyTask {
   long long sstride[3];    // stride (in doubles) in the SOURCE array when the dst index a increases by one (signed)
   long long sbase;         // source offset (doubles) of dst index (0,0,0) mapped
   double shift[3];         // coordinate shift (xyz fill only)
-  int pass;                // 1 faces, 2 edges, 3 corners
+  int pass;                // 1: all regions are filled by one launch (the chains are composed on the host)
+  int cta_begin;           // first CTA of this task in the flattened grid of the launch (prefix sum of the tasks' CTA counts)
 };
 
 struct BcTask {
@@ -121,6 +122,7 @@ struct RkFuse {
 
 // ---- kernel launchers (each enqueues on ctx->stream and bumps ctx->launches) --------------------
 int launch_fill_connect(cfd_ctx* c, int field /*0 q, 1 xyz*/);
+int fill_ctas_of(const CopyTask& T);   // CTAs of one ghost-fill task in the flattened grid
 int launch_bc_xyz(cfd_ctx* c);
 int launch_bc_q(cfd_ctx* c);
 int launch_metrics(cfd_ctx* c);

@@ -6,49 +6,61 @@
 
 // =================================================================================================
 // S6: ghost fill through signed index permutations (U15; P:L262 bc_block, "on GPU without
-// leaving the device").  One launch per pass (faces / edges / corners); blockIdx.y = task.
+// leaving the device").  One launch fills all regions (the face -> edge -> corner chains are composed on the host,
+// cfd_api.cu plan_copies); the grid is flattened over the tasks (CopyTask::cta_begin), FILL_CPT cells per thread.
 // =================================================================================================
+constexpr unsigned FILL_CPT = 2;   // cells per thread
+
 template <int NV, bool SHIFT>
-__global__ void __launch_bounds__(256) k_fill(const CopyTask* __restrict__ tasks, const BlockDev* __restrict__ blocks, int field) {
-  const CopyTask T = tasks[blockIdx.y];
+__global__ void __launch_bounds__(256) k_fill(const CopyTask* __restrict__ tasks, int ntasks, const BlockDev* __restrict__ blocks, int field) {
+  // flattened grid: CTA b belongs to the task with the largest cta_begin <= b (tasks are sorted by cta_begin)
+  int lo = 0, hi = ntasks - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (tasks[mid].cta_begin <= (int)blockIdx.x) lo = mid; else hi = mid - 1;
+  }
+  const CopyTask T = tasks[lo];
+  const unsigned cta = blockIdx.x - (unsigned)T.cta_begin;
   const long long cells = (long long)T.ext[0] * T.ext[1] * T.ext[2];
   const BlockDev D = blocks[T.dst_block];
   const BlockDev S = blocks[T.src_block];
   // no __restrict__: for a self-periodic block dst and src are the same buffer (disjoint regions within a pass)
   double* dst = field == 0 ? D.q : D.xyz;
   const double* src = field == 0 ? S.q : S.xyz;
-  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < cells; t += (long long)gridDim.x * blockDim.x) {
-    const int i = (int)(t % T.ext[0]);
-    const long long u = t / T.ext[0];
-    const int j = (int)(u % T.ext[1]);
-    const int k = (int)(u / T.ext[1]);
-    const int di = T.lo[0] + i, dj = T.lo[1] + j, dk = T.lo[2] + k;
+  // cells < 2^31 per region (a region is a ghost slab of one block): 32-bit index arithmetic
+  const unsigned e0 = (unsigned)T.ext[0], e1 = (unsigned)T.ext[1];
+  for (unsigned t = cta * (FILL_CPT * 256u) + threadIdx.x, n = 0; n < FILL_CPT && t < (unsigned)cells; ++n, t += 256u) {
+    const unsigned u = t / e0;
+    const int i = (int)(t - u * e0);
+    const unsigned k = u / e1;
+    const int j = (int)(u - k * e1);
+    const int di = T.lo[0] + i, dj = T.lo[1] + j, dk = T.lo[2] + (int)k;
     const long long od = D.idx(di, dj, dk);
     const long long os = T.sbase + di * T.sstride[0] + dj * T.sstride[1] + dk * T.sstride[2];
+    // all loads before the first store: dst and src may be the same buffer (no __restrict__), so the compiler would
+    // otherwise keep each load behind the previous store and leave one load in flight per thread
+    double val[NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      double val = src[v * S.M + os];
-      if (SHIFT) val += T.shift[v];
-      dst[v * D.M + od] = val;
-    }
+    for (int v = 0; v < NV; ++v) val[v] = src[v * S.M + os];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) dst[v * D.M + od] = SHIFT ? val[v] + T.shift[v] : val[v];
   }
+}
+
+int fill_ctas_of(const CopyTask& T) {
+  const long long cells = (long long)T.ext[0] * T.ext[1] * T.ext[2];
+  return (int)((cells + FILL_CPT * 256 - 1) / (FILL_CPT * 256));
 }
 
 int launch_fill_connect(cfd_ctx* c, int field) {
   for (int p = 1; p <= 3; ++p) {
     const size_t nt = c->tasks[p].size();
     if (!nt) continue;
-    long long mx = 0;
-    for (const CopyTask& T : c->tasks[p]) {
-      long long cells = (long long)T.ext[0] * T.ext[1] * T.ext[2];
-      if (cells > mx) mx = cells;
-    }
-    int gx = (int)((mx + 255) / 256);
-    if (gx > 2048) gx = 2048;
-    dim3 grid(gx, (unsigned)nt);
+    const CopyTask& L = c->tasks[p].back();
+    const unsigned ctas = (unsigned)(L.cta_begin + fill_ctas_of(L));
     ProfScope ps(c, PK_FILL);
-    if (field == 0) k_fill<5, false><<<grid, 256, 0, c->stream>>>(c->d_tasks[p], c->d_blocks, 0);
-    else k_fill<3, true><<<grid, 256, 0, c->stream>>>(c->d_tasks[p], c->d_blocks, 1);
+    if (field == 0) k_fill<5, false><<<ctas, 256, 0, c->stream>>>(c->d_tasks[p], (int)nt, c->d_blocks, 0);
+    else k_fill<3, true><<<ctas, 256, 0, c->stream>>>(c->d_tasks[p], (int)nt, c->d_blocks, 1);
     c->launches++;
   }
   CUDA_TRY(c, cudaGetLastError());
