@@ -107,6 +107,27 @@ int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cf
                       const cfd_face* faces, const cfd_params* params, void* workspace, size_t workspace_bytes,
                       void* cuda_stream);
 
+/* NEXT-4 (the paper shards one sub-block set per GPU and exchanges halos over MPI / GPUDirect P2P on
+ * PCIe): BLOCK SHARDING over the GPUs of one NVLink / NVSwitch node, one process per
+ * GPU.  The same call as cfd_create_blocks over the WHOLE topology (all nblocks blocks, all faces), but this context
+ * OWNS only the blocks with local[b] != 0 (local == NULL: all of them); the others are advanced by peer processes.
+ * For a peer's block, ptrs[b].q, .qn, .r, .xyz are PEER-MAPPED device pointers to that process's buffers (CUDA IPC /
+ * P2P over NVLink; khat, jac may be NULL), given in the same order as the owner passed them, and are only ever READ:
+ * cfd_exchange_interfaces (and the xyz fill of cfd_compute_metrics) pull the ghost layers of the local blocks straight
+ * out of the owner's interior cells with P2P loads through the same composed index maps -- no packing, no staging
+ * buffer, no host copy (on NVSwitch every peer is equidistant, so the paper's topology-aware placement, P:L356–390,
+ * has nothing left to decide).  Everything else (metrics, RHS, RK stage, BCs, CFL, step_host) runs on the local blocks
+ * only; res5 and the CFL maximum are LOCAL sums / maxima: the caller reduces them over the processes.
+ * Ordering is the caller's job (the binding does it with collectives on the compute stream): every process must have
+ * finished the stage's last sweep before any process runs cfd_exchange_interfaces of that stage, all processes must call
+ * the stage functions in lock step (the buffer roles of cfd_stage_fused rotate identically everywhere), and the
+ * owners' xyz interiors must be in place before cfd_compute_metrics.  The workspace is sized by
+ * cfd_workspace_bytes_sharded (local blocks only). */
+int cfd_create_blocks_sharded(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cfd_block_ptrs* ptrs, const int* local,
+                              int nfaces, const cfd_face* faces, const cfd_params* params, void* workspace,
+                              size_t workspace_bytes, void* cuda_stream);
+size_t cfd_workspace_bytes_sharded(int nblocks, const cfd_dims* dims, const int* local, const cfd_params* params);
+
 /* S1 (Eqs. 7–8): fills the ghost layers of xyz (interfaces / periodic shift, wall = odd
  * reflection, far field = linear extrapolation), then khat and jac by 6th-order central differences
  * in conservative form, valid on the index box [-3, n+3)^3 of every block.
@@ -154,6 +175,12 @@ int cfd_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
  * (cfd_rhs, cfd_rk_stage, cfd_exchange_interfaces, cfd_apply_bc, cfd_step_host) follows the current roles.
  * The contents of the r buffer after this call are scratch.  res5_host_or_null as in cfd_rk_stage. */
 int cfd_stage_fused(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
+
+/* The part of cfd_stage_fused that touches the context's own blocks only: S2 + S3 with S4 inside the last sweep and the
+ * exchange of the buffer roles, WITHOUT the ghost fill and the physical BCs.  A sharded context (cfd_create_blocks_sharded)
+ * calls this, lets every process reach the same point (a collective on the compute stream), and then calls
+ * cfd_exchange_interfaces and cfd_apply_bc; on an unsharded context the three calls in a row are cfd_stage_fused. */
+int cfd_stage_fused_local(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
 
 /* roles[0], roles[1], roles[2] = which buffer of cfd_block_ptrs (0 = the one passed as q, 1 = qn, 2 = r)
  * currently holds Q, Q^n and R / scratch.  (0, 1, 2) until cfd_stage_fused or cfd_step_host is used. */

@@ -20,7 +20,7 @@ ABI_SYMBOLS = (
     "cfd_exchange_interfaces", "cfd_apply_bc", "cfd_stage", "cfd_destroy", "cfd_last_error",
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
     "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan", "cfd_stage_fused", "cfd_buffer_roles",
-    "cfd_cfl_dt",
+    "cfd_cfl_dt", "cfd_create_blocks_sharded", "cfd_workspace_bytes_sharded", "cfd_stage_fused_local",
 )
 PROF_NCLASS = 12
 
@@ -66,7 +66,12 @@ def _load():
         getattr(L, n).argtypes = [C.c_void_p]
     L.cfd_buffer_roles.restype = C.c_int
     L.cfd_buffer_roles.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
-    for n in ("cfd_rk_stage", "cfd_stage", "cfd_stage_fused"):
+    L.cfd_workspace_bytes_sharded.restype = C.c_size_t
+    L.cfd_workspace_bytes_sharded.argtypes = [C.c_int, C.POINTER(_Dims), C.POINTER(C.c_int), C.POINTER(_Params)]
+    L.cfd_create_blocks_sharded.restype = C.c_int
+    L.cfd_create_blocks_sharded.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(_Dims), C.POINTER(_Ptrs), C.POINTER(C.c_int),
+                                            C.c_int, C.POINTER(_Face), C.POINTER(_Params), C.c_void_p, C.c_size_t, C.c_void_p]
+    for n in ("cfd_rk_stage", "cfd_stage", "cfd_stage_fused", "cfd_stage_fused_local"):
         getattr(L, n).restype = C.c_int
         getattr(L, n).argtypes = [C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_double)]
     L.cfd_cfl_dt.restype = C.c_int

@@ -12,10 +12,14 @@ static inline bool is_connect(int t) { return t == CFD_FACE_PERIODIC || t == CFD
 size_t ws_partials_offset_doubles(const cfd_ctx* c) { return (size_t)WS_ROWS * (size_t)c->sum_M + 8; }  // + 8: past the shifted scratch rows
 int rk_max_partial_blocks() { return 16384; }
 
-extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params*) {
-  long long sum = 0;  // every block has its own WS_ROWS M doubles (the blocks' kernels run concurrently on side streams)
-  for (int b = 0; b < nblocks; ++b) sum += (long long)(dims[b].ni + 2 * NG) * (dims[b].nj + 2 * NG) * (dims[b].nk + 2 * NG);
+extern "C" size_t cfd_workspace_bytes_sharded(int nblocks, const cfd_dims* dims, const int* local, const cfd_params*) {
+  long long sum = 0;  // every LOCAL block has its own WS_ROWS M doubles (the blocks' kernels run concurrently on side streams)
+  for (int b = 0; b < nblocks; ++b)
+    if (!local || local[b]) sum += (long long)(dims[b].ni + 2 * NG) * (dims[b].nj + 2 * NG) * (dims[b].nk + 2 * NG);
   return ((size_t)WS_ROWS * (size_t)sum + (size_t)rk_max_partial_blocks() * 5 * (size_t)(nblocks > 0 ? nblocks : 1) + 64) * sizeof(double);
+}
+extern "C" size_t cfd_workspace_bytes(int nblocks, const cfd_dims* dims, const cfd_params* prm) {
+  return cfd_workspace_bytes_sharded(nblocks, dims, nullptr, prm);
 }
 
 // the six assignments of three buffers to the roles (q, qn, r): id -> role[]
@@ -100,6 +104,7 @@ static void plan_copies(cfd_ctx* c) {
     fidx[(size_t)c->faces[t].block * 6 + c->faces[t].face] = (int)t;
   }
   for (size_t b = 0; b < nb; ++b) {
+    if (!c->is_local(b)) continue;  // a peer GPU fills the ghost layers of its own blocks
     const BlockDev& B = c->blk[b];
     for (int code = 0; code < 27; ++code) {
       int side[3] = {code % 3, (code / 3) % 3, code / 9};  // 0 below, 1 inside, 2 above
@@ -142,6 +147,12 @@ static void plan_copies(cfd_ctx* c) {
 extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cfd_block_ptrs* ptrs, int nfaces,
                                  const cfd_face* faces, const cfd_params* params, void* workspace, size_t workspace_bytes,
                                  void* cuda_stream) {
+  return cfd_create_blocks_sharded(out, nblocks, dims, ptrs, nullptr, nfaces, faces, params, workspace, workspace_bytes, cuda_stream);
+}
+
+extern "C" int cfd_create_blocks_sharded(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cfd_block_ptrs* ptrs, const int* local,
+                                         int nfaces, const cfd_face* faces, const cfd_params* params, void* workspace,
+                                         size_t workspace_bytes, void* cuda_stream) {
   if (!out || nblocks < 1 || !dims || !ptrs || !params || nfaces < 0 || (nfaces > 0 && !faces))
     return fail_create(CFD_E_ARG, "cfd_create_blocks: null argument or nblocks < 1");
   *out = nullptr;
@@ -165,6 +176,12 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
   for (int m = 0; m < 5; ++m) c->pd.q_inf[m] = params->q_inf[m];
   c->stream = (cudaStream_t)cuda_stream;
   c->blk.resize(nblocks);
+  if (local) {
+    c->local.assign(local, local + nblocks);
+    bool any = false;
+    for (int b = 0; b < nblocks; ++b) any = any || local[b];
+    if (!any) { delete c; return fail_create(CFD_E_ARG, "cfd_create_blocks_sharded: this context owns no block"); }
+  }
   for (int b = 0; b < nblocks; ++b) {
     BlockDev& B = c->blk[b];
     B.n[0] = dims[b].ni; B.n[1] = dims[b].nj; B.n[2] = dims[b].nk;
@@ -176,8 +193,9 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
     B.s[0] = 1; B.s[1] = B.m[0]; B.s[2] = (long long)B.m[0] * B.m[1];
     B.q = ptrs[b].q; B.qn = ptrs[b].qn; B.r = ptrs[b].r; B.xyz = ptrs[b].xyz; B.khat = ptrs[b].khat; B.jac = ptrs[b].jac;
     const void* pp[6] = {B.q, B.qn, B.r, B.xyz, B.khat, B.jac};
-    for (int t = 0; t < 6; ++t)
+    for (int t = 0; t < (c->is_local(b) ? 6 : 4); ++t)  // a peer's block: q, qn, r, xyz (peer-mapped) only
       if (!pp[t] || ((uintptr_t)pp[t] & 15u)) { delete c; return fail_create(CFD_E_ARG, "cfd_create_blocks: null or misaligned (16 B) field pointer"); }
+    if (!c->is_local(b)) continue;
     if (B.M > c->max_M) c->max_M = B.M;
     c->sum_M += B.M;
   }
@@ -209,7 +227,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
       if (F.type == CFD_FACE_WALL_NOSLIP_ADIABATIC && c->blk[F.block].n[F.face / 2] < NG + 1)
         return bad("a wall needs at least 7 interior nodes along its normal");
       BcTask T{F.block, F.face, F.type};
-      c->bcs.push_back(T);
+      if (c->is_local(F.block)) c->bcs.push_back(T);
     } else {
       return bad("unknown face type");
     }
@@ -238,7 +256,7 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
     }
   }
   // ---- workspace ----
-  size_t need = cfd_workspace_bytes(nblocks, dims, params);
+  size_t need = cfd_workspace_bytes_sharded(nblocks, dims, local, params);
   if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 15u)) {
     delete c;
     return fail_create(CFD_E_WORKSPACE, "cfd_create_blocks: workspace null, misaligned or smaller than cfd_workspace_bytes()");
@@ -249,7 +267,12 @@ extern "C" int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dim
     long long off = 0;
     // + 2: the scratch rows are indexed like the fields but shifted by two doubles, so that interior i = 0 (array index NG = 6)
     // starts a 32-byte sector: the rows are written in interior runs, and half-sector writes cost a read-modify-write
-    for (BlockDev& B : c->blk) { B.ws = c->ws + (long long)WS_ROWS * off + 2; off += B.M; }
+    for (size_t b = 0; b < c->blk.size(); ++b) {
+      BlockDev& B = c->blk[b];
+      if (!c->is_local(b)) { B.ws = nullptr; continue; }
+      B.ws = c->ws + (long long)WS_ROWS * off + 2;
+      off += B.M;
+    }
   }
   plan_copies(c);
   // ---- small device-side descriptor arrays (a few KB; the only allocations the library makes) ----
@@ -355,7 +378,7 @@ extern "C" int cfd_cfl_dt(cfd_ctx* c, double cfl, double* dt_host, double* const
   if (!(cfl > 0.0)) { c->err = "cfd_cfl_dt: cfl must be > 0"; return CFD_E_ARG; }
   if (dt_local)
     for (size_t b = 0; b < c->blk.size(); ++b)
-      if (!dt_local[b] || ((uintptr_t)dt_local[b] & 7u)) { c->err = "cfd_cfl_dt: null or misaligned dt_local pointer"; return CFD_E_ARG; }
+      if (c->is_local(b) && (!dt_local[b] || ((uintptr_t)dt_local[b] & 7u))) { c->err = "cfd_cfl_dt: null or misaligned dt_local pointer"; return CFD_E_ARG; }
   int rc = launch_cfl(c, cfl, dt_local);
   if (rc != 0) return rc;
   double smax = 0.0;
@@ -384,7 +407,7 @@ extern "C" int cfd_stage(cfd_ctx* c, int stage, double dt, double* res5) {
   return cfd_apply_bc(c);
 }
 
-extern "C" int cfd_stage_fused(cfd_ctx* c, int stage, double dt, double* res5) {
+extern "C" int cfd_stage_fused_local(cfd_ctx* c, int stage, double dt, double* res5) {
   if (!c) return CFD_E_ARG;
   if (stage < 1 || stage > 3) { c->err = "cfd_stage_fused: stage must be 1..3"; return CFD_E_STAGE; }
   int rc = launch_rhs(c, stage, dt);
@@ -396,6 +419,12 @@ extern "C" int cfd_stage_fused(cfd_ctx* c, int stage, double dt, double* res5) {
     CUDA_TRY(c, cudaMemcpyAsync(res5, c->d_res, 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   }
+  return CFD_OK;
+}
+
+extern "C" int cfd_stage_fused(cfd_ctx* c, int stage, double dt, double* res5) {
+  int rc = cfd_stage_fused_local(c, stage, dt, res5);
+  if (rc != 0) return rc;
   if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
   return cfd_apply_bc(c);
 }
@@ -421,6 +450,7 @@ extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const
     return cudaMemcpy3DAsync(&p, c->stream);
   };
   for (size_t b = 0; b < c->blk.size(); ++b) {
+    if (!c->is_local(b)) continue;
     const BlockDev& B = c->blk[b];
     if (!qin[b] || !qout[b]) { c->err = "cfd_step_host: null host pointer"; return CFD_E_ARG; }
     const size_t N = (size_t)B.n[0] * B.n[1] * B.n[2];
@@ -433,6 +463,7 @@ extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const
   for (int s = 1; s <= 3; ++s)
     if ((rc = cfd_stage_fused(c, s, dt, nullptr)) != 0) return rc;
   for (size_t b = 0; b < c->blk.size(); ++b) {
+    if (!c->is_local(b)) continue;
     const BlockDev& B = c->blk[b];
     const size_t N = (size_t)B.n[0] * B.n[1] * B.n[2];
     ProfScope ps(c, PK_COPY);

@@ -269,7 +269,9 @@ __global__ void __launch_bounds__(256) k_metric_khat(BlockDev B, const double* _
 }
 
 int launch_metrics(cfd_ctx* c) {
-  for (const BlockDev& B : c->blk) {
+  for (size_t b = 0; b < c->blk.size(); ++b) {
+    if (!c->is_local(b)) continue;
+    const BlockDev& B = c->blk[b];
     ProfScope ps(c, PK_METRICS);
     k_metric_d1<<<(unsigned)((B.M + 255) / 256), 256, 0, c->stream>>>(B, B.ws);
     const long long box = (long long)(B.n[0] + 6) * (B.n[1] + 6) * (B.n[2] + 6);
@@ -343,7 +345,9 @@ int launch_rk(cfd_ctx* c, int stage, double dt) {
   const double b = stage == 1 ? 1.0 : (stage == 2 ? 1.0 / 4.0 : 2.0 / 3.0);
   double* partials = c->ws + ws_partials_offset_doubles(c);
   int used = 0;
-  for (const BlockDev& B : c->blk) {
+  for (size_t bi = 0; bi < c->blk.size(); ++bi) {
+    if (!c->is_local(bi)) continue;
+    const BlockDev& B = c->blk[bi];
     const long long N = (long long)B.n[0] * B.n[1] * B.n[2];
     long long g = (N + 255) / 256;
     const int cap = rk_max_partial_blocks();

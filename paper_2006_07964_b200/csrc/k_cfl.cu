@@ -63,6 +63,7 @@ int launch_cfl(cfd_ctx* c, double cfl, double* const* dt_local) {
   int used = 0;
   const int cap = rk_max_partial_blocks();
   for (size_t b = 0; b < c->blk.size(); ++b) {
+    if (!c->is_local(b)) continue;
     const BlockDev& B = c->blk[b];
     const long long N = (long long)B.n[0] * B.n[1] * B.n[2];
     long long g = (N + CT - 1) / CT;

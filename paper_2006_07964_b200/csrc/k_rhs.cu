@@ -48,15 +48,19 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
   // kernels goes to one of the library-owned side streams, forked from and joined back into the context's stream, so that
   // small blocks (C4: 8 x 96^3, about one wave of CTAs per kernel) fill the GPU together.  Every block has its own scratch.
   cudaStream_t const main_stream = c->stream;
-  const bool fork = c->blk.size() > 1 && !c->prof_on && c->side[0] != nullptr;
+  size_t nlocal = 0;
+  for (size_t b = 0; b < c->blk.size(); ++b) nlocal += c->is_local(b) ? 1 : 0;
+  const bool fork = nlocal > 1 && !c->prof_on && c->side[0] != nullptr;
   if (fork) {
     CUDA_TRY(c, cudaEventRecord(c->ev_fork, main_stream));
     for (int t = 0; t < cfd_ctx::NSIDE; ++t) CUDA_TRY(c, cudaStreamWaitEvent(c->side[t], c->ev_fork, 0));
   }
   int bi = 0, rc = 0;
   // the sweeps size their segments for the CTAs of all concurrently running blocks (C4: 3.31 -> 3.48 Gpts/s)
-  c->conc = fork ? (int)(c->blk.size() < (size_t)cfd_ctx::NSIDE ? c->blk.size() : (size_t)cfd_ctx::NSIDE) : 1;
-  for (const BlockDev& B : c->blk) {
+  c->conc = fork ? (int)(nlocal < (size_t)cfd_ctx::NSIDE ? nlocal : (size_t)cfd_ctx::NSIDE) : 1;
+  for (size_t bx = 0; bx < c->blk.size(); ++bx) {
+    if (!c->is_local(bx)) continue;  // NEXT-4: a peer GPU advances this block
+    const BlockDev& B = c->blk[bx];
     if (fork) c->stream = c->side[bi++ % cfd_ctx::NSIDE];
     if (c->pd.viscous) {
       ProfScope ps(c, PK_VISC_FLUX);

@@ -497,7 +497,7 @@ void xi_tma_setup(cfd_ctx* c) {
   for (size_t b = 0; b < c->blk.size(); ++b) {
     const BlockDev& B = c->blk[b];
     XiMaps& X = S->maps[b];
-    if ((B.m[0] & 1) || B.n[0] < 8) continue;
+    if ((B.m[0] & 1) || B.n[0] < 8 || !c->is_local(b)) continue;
     bool ok = true;
     for (int t = 0; t < 3; ++t) ok = ok && encode(fn, &X.st[t], B, c->base[t][b], 5);
     ok = ok && encode(fn, &X.kh, B, B.khat, 3);
