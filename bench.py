@@ -392,6 +392,114 @@ def measure_gpu(name, steps, warmup, device, dist=None, e2e=True, profile=True, 
     return out
 
 
+def measure_sharded(name, steps, warmup, device, dist, repeats):
+    """NEXT-4 (--sharded): the blocks of the workload are partitioned over the ranks (one process per GPU), every rank
+    advances its own blocks and pulls its ghost layers from the peers' memory over NVLink (sharded.py).  Same timing
+    protocol as measure_gpu; the job's work is FIXED (strong scaling).  Returns ms per repeat (max over ranks)."""
+    import torch
+
+    from paper_2006_07964_b200.sharded import Comm, ShardedContext, halo_bytes_per_stage, partition_blocks
+
+    case = make_case(name)
+    world = dist.get_world_size() if dist is not None else 1
+    rank = dist.get_rank() if dist is not None else 0
+    owner = partition_blocks(case.dims, world)
+    comm = Comm(dist, device) if dist is not None else None
+    ctx = ShardedContext(case.dims, case.faces, case.params, owner, comm, device=device)
+    ctx.load_case(case)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(device)
+
+    for _ in range(warmup):
+        ctx.step(case.dt)
+    barrier()
+    didx = torch.device(device).index or 0
+    sampler = ClockSampler("GPU-" + str(torch.cuda.get_device_properties(didx).uuid))
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0, rep_ms = ctx.launch_count, []
+    for _ in range(max(1, repeats)):
+        barrier()
+        e0.record(ctx.stream)
+        for _ in range(steps):
+            ctx.step(case.dt)
+        e1.record(ctx.stream)
+        barrier()
+        rep_ms.append(max_over_ranks(e0.elapsed_time(e1), dist, device))
+    launches = (ctx.launch_count - l0) // max(1, repeats)
+    clocks = sampler.stop()
+    finite = bool(all(torch.isfinite(ctx.interior(b, "q")).all().item() for b in ctx.local))
+    # end to end: pinned host buffers of the local blocks in and out every step
+    qh = {b: torch.empty((5,) + tuple(reversed(case.dims[b])), dtype=torch.float64).pin_memory() for b in ctx.local}
+    for b in ctx.local:
+        qh[b].copy_(ctx.interior(b, "q"))
+    ctx.step_host(qh, qh, case.dt)
+    barrier()
+    e0.record(ctx.stream)
+    for _ in range(steps):
+        ctx.step_host(qh, qh, case.dt)
+    e1.record(ctx.stream)
+    barrier()
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1), dist, device)
+    nbytes = sum(q.numel() * 8 for q in qh.values())
+    out = dict(ms=float(np.median(rep_ms)), rep_ms=rep_ms, pts=case.npoints, launches=launches, clocks=clocks, finite=finite,
+               owner=owner, halo=halo_bytes_per_stage(case.dims, case.faces, owner, rank), dims=case.dims, params=dict(case.params),
+               dt=case.dt, e2e=dict(ms=e2e_ms, h2d=nbytes, d2h=nbytes))
+    ctx.close()
+    return out
+
+
+def run_sharded(args):
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    device = f"cuda:{local}"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist_mod.init_process_group(backend="nccl", device_id=torch.device(device))
+        dist = dist_mod
+    hbm_gbs, _ = load_peaks()
+    m = measure_sharded(args.workload, args.steps, args.warmup, device, dist, args.repeats)
+    if rank == 0:
+        pts, visc = m["pts"], int(m["params"]["viscous"])
+        value = pts * 3 * args.steps / (m["ms"] * 1e-3) / 1e9          # the job's points are fixed: NOT multiplied by world
+        flop_stage = FLOPS_PER_POINT["ns_stage" if visc else "euler_stage"]
+        roof = world / max(flop_stage / (FP64_PEAK_NOMINAL_TFLOPS * 1e12), BYTES_PER_POINT_STAGE / (hbm_gbs * 1e9)) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": m["ms"] / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.workload], "name": args.workload, "blocks": len(m["dims"]), "points": pts,
+                       "stages_per_step": 3, "viscous": visc, "scheme": 0, "dt": m["dt"],
+                       "parallelism": f"blocks sharded over {world} GPU(s), ghost layers pulled from the peers by P2P loads "
+                                      "(NEXT-4, sharded.py)",
+                       "owner": m["owner"], "halo_bytes_pulled_per_stage_rank0": m["halo"]},
+            "timing": {"repeats": args.repeats, "ms_per_step_each_repeat": [x / args.steps for x in m["rep_ms"]]},
+            "state_finite": m["finite"],
+            "stage_roofline": {"roofline_gpts": roof, "frac": value / roof, "flop_per_point_stage": flop_stage},
+            "roofline": None, "cpu_baseline": None,
+            "e2e": {"value": pts * 3 * args.steps / (m["e2e"]["ms"] * 1e-3) / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": m["e2e"]["h2d"], "d2h_bytes_per_step": m["e2e"]["d2h"],
+                    "ms_per_step": m["e2e"]["ms"] / args.steps},
+            "gpu_launches": m["launches"], "clocks": m["clocks"],
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 class _CaseView:
     """What kernel_rooflines needs of a case (the arrays themselves are released after the measurement)."""
 
@@ -530,9 +638,13 @@ def main():
     ap.add_argument("--no-also", action="store_true")
     ap.add_argument("--plan", type=int, default=0, help="cfd_set_sweep_plan (0 default; 1 all tiled; 2 all marching)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sharded", action="store_true",
+                    help="NEXT-4: shard the blocks of a multi-block workload over the ranks (strong scaling) instead of replicas")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.sharded:
+        run_sharded(args)
     else:
         run_ours(args)
 

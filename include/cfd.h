@@ -203,6 +203,11 @@ int cfd_profile_enable(cfd_ctx*, int on);
 int cfd_profile_read(cfd_ctx*, double ms[CFD_PROF_NCLASS], long long launches[CFD_PROF_NCLASS]);
 const char* cfd_profile_name(int id);
 
+/* Measurement aid (power / clock measurements of one kernel class looped alone, profiles/r2_power.md): cfd_rhs and
+ * cfd_stage_fused launch only the hot kernel classes whose bit (1 << class id: 0 xi sweep, 1 eta sweep, 2 zeta sweep,
+ * 3 viscous point fluxes) is set in mask.  With any of these bits clear the RESULTS ARE INVALID; the default is all ones. */
+int cfd_profile_only(cfd_ctx*, unsigned mask);
+
 /* Frees the context (never the caller's buffers). */
 int cfd_destroy(cfd_ctx*);
 

@@ -502,6 +502,12 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
   return CFD_OK;
 }
 
+extern "C" int cfd_profile_only(cfd_ctx* c, unsigned mask) {
+  if (!c) return CFD_E_ARG;
+  c->only_mask = mask;
+  return CFD_OK;
+}
+
 extern "C" int cfd_set_sweep_plan(cfd_ctx* c, int plan) {
   if (!c) return CFD_E_ARG;
   if (plan != 0 && plan != 4 && plan != 5) { c->err = "cfd_set_sweep_plan: plan must be 0, 4 or 5"; return CFD_E_ARG; }

@@ -79,6 +79,7 @@ struct cfd_ctx {
   cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
   int conc = 1;                       // blocks whose kernel chains run concurrently (side streams): the sweeps size their segments for conc x their own CTAs
   long long launches = 0;
+  unsigned only_mask = 0xffffffffu;  // cfd_profile_only: kernel classes (bit = ProfClass id) that launch_rhs still launches
   int xi_mode = 0;                    // xi kernel (cfd_set_sweep_plan): 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
   std::string err;
   // per-kernel event timing (cfd_profile_*): event pairs in launch order, reused after each read

@@ -19,7 +19,7 @@ int sweep_init() { return march_init(); }
 // k_xi_ldg and, for odd ni, the plain marching kernel with strided lanes.
 static int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* rk_ctas) {
   int rc = 0;
-  {
+  if (c->only_mask & (1u << PK_INV_XI)) {
     ProfScope ps(c, PK_INV_XI);
     const int b = (int)(&B - c->blk.data());
     const bool orig = c->prm.scheme == 1;
@@ -28,8 +28,8 @@ static int launch_sweeps(cfd_ctx* c, const BlockDev& B, const RkFuse* rk, int* r
     else if (orig) rc = launch_march(c, B, 0, 0, nullptr, nullptr, false, true);
     else rc = launch_march_xi(c, B);
   }
-  if (rc == 0) { ProfScope ps(c, PK_INV_ETA); rc = launch_march(c, B, 1, 1, nullptr, nullptr, true, false); }
-  if (rc == 0) { ProfScope ps(c, PK_INV_ZETA); rc = launch_march(c, B, 2, 2, rk, rk_ctas, false, false); }
+  if (rc == 0 && (c->only_mask & (1u << PK_INV_ETA))) { ProfScope ps(c, PK_INV_ETA); rc = launch_march(c, B, 1, 1, nullptr, nullptr, true, false); }
+  if (rc == 0 && (c->only_mask & (1u << PK_INV_ZETA))) { ProfScope ps(c, PK_INV_ZETA); rc = launch_march(c, B, 2, 2, rk, rk_ctas, false, false); }
   return rc;
 }
 
@@ -62,7 +62,7 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
     if (!c->is_local(bx)) continue;  // NEXT-4: a peer GPU advances this block
     const BlockDev& B = c->blk[bx];
     if (fork) c->stream = c->side[bi++ % cfd_ctx::NSIDE];
-    if (c->pd.viscous) {
+    if (c->pd.viscous && (c->only_mask & (1u << PK_VISC_FLUX))) {
       ProfScope ps(c, PK_VISC_FLUX);
       rc = launch_visc_march(c, B);
     }

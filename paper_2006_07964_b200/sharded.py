@@ -295,6 +295,24 @@ class ShardedContext:
                 res = r
         return res
 
+    def step_host(self, q_in, q_out, dt):
+        """End to end with HOST buffers: {block: pinned host tensor (5, nk, nj, ni)} for the local blocks in, one RK3 step,
+        the same out (may alias); the copies ride on the compute stream, the call returns after a synchronise."""
+        t = self.torch
+        with t.cuda.stream(self.stream):
+            for b in self.local:
+                self.interior(b, "q").copy_(q_in[b], non_blocking=True)
+        self._barrier()
+        self.exchange()
+        if self.has_bc:
+            self._barrier()
+            self.apply_bc()
+        self.step(dt)
+        with t.cuda.stream(self.stream):
+            for b in self.local:
+                q_out[b].copy_(self.interior(b, "q"), non_blocking=True)
+        self.stream.synchronize()
+
     def cfl_dt(self, cfl):
         """min over the ranks of the local cfd_cfl_dt."""
         dt = C.c_double()
