@@ -612,3 +612,23 @@ def test_shock_vortex_fifty_steps(po, W, B, which):
     rho = qo[0]
     assert (np.abs(np.diff(rho, axis=2)) / rho[:, :, 1:]).max() > 0.15
     assert_rhs_parity(o, g, case)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# cfd_profile_only: the measurement aid of profiles/r2_power.md (one kernel class looped alone)
+# ---------------------------------------------------------------------------------------------------------------------
+def test_profile_only_masks_kernel_classes_and_default_restores_parity(po, W, B):
+    case = W.c3_tgv(24)
+    o, g = pair(po, B, case)
+    g.field(0, "r").fill_(-7.0)
+    n0 = g.launch_count
+    g.profile_only(0)               # nothing of the hot classes runs: r stays untouched
+    g.rhs()
+    assert g.launch_count == n0
+    assert float(g.interior(0, "r").min()) == -7.0 and float(g.interior(0, "r").max()) == -7.0
+    g.profile_only(1 << 0)          # the xi sweep alone: one launch, r = X^xi only (not the RHS)
+    g.rhs()
+    assert g.launch_count == n0 + 1
+    assert float(g.interior(0, "r").abs().max()) != 7.0
+    g.profile_only()                # default: all classes, and the RHS meets the oracle again
+    assert_rhs_parity(o, g, case)
