@@ -18,7 +18,7 @@
  *    carrying CFD_NG = 6 ghost layers on both sides: extents (ni+12, nj+12, nk+12),
  *    M = (ni+12)(nj+12)(nk+12) doubles per variable.  Pointers must be 16-byte aligned.
  *  - All work is ordered on the CUDA stream given to cfd_create_blocks: it is enqueued there or, for contexts
- *    with more than one block, partly on four library-owned non-blocking side streams that cfd_rhs /
+ *    with more than one block, partly on eight library-owned non-blocking side streams that cfd_rhs /
  *    cfd_stage_fused fork from that stream and join back into it before they return (the blocks' kernel chains
  *    run concurrently; work enqueued on the caller's stream before or after a call is ordered with it).  No
  *    function synchronises the device unless documented ("returns host values").

@@ -74,9 +74,9 @@ struct cfd_ctx {
   size_t ws_bytes = 0;
   long long max_M = 0;
   long long sum_M = 0;                // sum of M over the blocks: the per-block scratch areas are WS_ROWS M doubles each
-  static constexpr int NSIDE = 4;     // side streams: the blocks of a multi-block case run their per-block kernels concurrently
-  cudaStream_t side[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
-  cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {nullptr, nullptr, nullptr, nullptr};
+  static constexpr int NSIDE = 8;     // side streams: the blocks of a multi-block case run their per-block kernels concurrently
+  cudaStream_t side[NSIDE] = {};
+  cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {};
   int conc = 1;                       // blocks whose kernel chains run concurrently (side streams): the sweeps size their segments for conc x their own CTAs
   long long launches = 0;
   unsigned only_mask = 0xffffffffu;  // cfd_profile_only: kernel classes (bit = ProfClass id) that launch_rhs still launches
