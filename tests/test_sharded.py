@@ -233,3 +233,18 @@ def test_sharded_two_processes_cuda_ipc_on_one_gpu(W):
         assert np.allclose(res, res1, rtol=1e-13, atol=0.0)   # all-reduced over the two ranks
         assert dt == dt1
     assert seen == set(range(8))
+
+
+@pytest.mark.gpu
+def test_bench_sharded_line_on_one_gpu():
+    """`bench.py --sharded` at N = 1 (all blocks local, nothing pulled): the JSON line of the sharded arm."""
+    import json
+    import subprocess
+
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--sharded", "--workload", "c4", "--steps", "2", "--warmup", "3",
+                        "--repeats", "1"], capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads([ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1])
+    assert d["scaling"] == "strong" and d["n_gpus"] == 1 and d["unit"] == "Gpts/s"
+    assert d["config"]["owner"] == [0] * 8 and d["config"]["halo_bytes_pulled_per_stage_rank0"] == 0
+    assert d["state_finite"] and d["value"] > 0.5 and d["e2e"]["value"] > 0 and d["gpu_launches"] > 0
