@@ -235,6 +235,11 @@ int cfd_fp64_peak_probe(int iters, double* tflops);
  * retired after profiles/r1_*.md settled the comparison. */
 int cfd_set_sweep_plan(cfd_ctx*, int plan);
 
+/* Tile of the viscous point-flux kernel (k_visc_march; all choices compute the same values bit for bit): -1 (default) picks,
+ * per block, the geometry with the fewest thread-planes; 0 = 64 x 8 threads (58 output columns per tile row), 1 = 70 x 7
+ * (64 columns), 2 = 54 x 9 (48 columns).  For tests and measurements. */
+int cfd_set_visc_tile(cfd_ctx*, int tile);
+
 /* Device self-test of the branch-free fp64 reciprocal / reciprocal square root the hot kernels use instead
  * of IEEE division (csrc/fastmath.cuh): for n HOST values x > 0 writes 1/x and 1/sqrt(x) as the kernels compute
  * them into the HOST arrays rcp_out, rsqrt_out (tests compare with correctly rounded results).  Allocates

@@ -21,7 +21,7 @@ ABI_SYMBOLS = (
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
     "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan", "cfd_stage_fused", "cfd_buffer_roles",
     "cfd_cfl_dt", "cfd_create_blocks_sharded", "cfd_workspace_bytes_sharded", "cfd_stage_fused_local",
-    "cfd_profile_only",
+    "cfd_profile_only", "cfd_set_visc_tile",
 )
 PROF_NCLASS = 12
 
@@ -89,6 +89,8 @@ def _load():
     L.cfd_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.cfd_profile_name.restype = C.c_char_p
     L.cfd_profile_name.argtypes = [C.c_int]
+    L.cfd_set_visc_tile.restype = C.c_int
+    L.cfd_set_visc_tile.argtypes = [C.c_void_p, C.c_int]
     L.cfd_profile_only.restype = C.c_int
     L.cfd_profile_only.argtypes = [C.c_void_p, C.c_uint]
     L.cfd_set_sweep_plan.restype = C.c_int
@@ -294,6 +296,9 @@ class Context:
 
     def set_sweep_plan(self, plan):
         self._chk(lib.cfd_set_sweep_plan(self.h, int(plan)))
+
+    def set_visc_tile(self, tile=-1):
+        self._chk(lib.cfd_set_visc_tile(self.h, int(tile)))
 
     def profile_only(self, mask=0xFFFFFFFF):
         """cfd_profile_only: launch only the hot kernel classes in mask (measurement aid; results invalid unless all ones)."""

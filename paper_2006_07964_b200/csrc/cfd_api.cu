@@ -502,6 +502,13 @@ extern "C" int cfd_profile_read(cfd_ctx* c, double* ms, long long* launches) {
   return CFD_OK;
 }
 
+extern "C" int cfd_set_visc_tile(cfd_ctx* c, int tile) {
+  if (!c) return CFD_E_ARG;
+  if (tile < -1 || tile > 2) { c->err = "cfd_set_visc_tile: tile must be -1 (automatic), 0, 1 or 2"; return CFD_E_ARG; }
+  c->visc_tile = tile;
+  return CFD_OK;
+}
+
 extern "C" int cfd_profile_only(cfd_ctx* c, unsigned mask) {
   if (!c) return CFD_E_ARG;
   c->only_mask = mask;

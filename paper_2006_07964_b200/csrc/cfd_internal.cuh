@@ -79,6 +79,7 @@ struct cfd_ctx {
   cudaEvent_t ev_fork = nullptr, ev_join[NSIDE] = {};
   int conc = 1;                       // blocks whose kernel chains run concurrently (side streams): the sweeps size their segments for conc x their own CTAs
   long long launches = 0;
+  int visc_tile = -1;                 // cfd_set_visc_tile: -1 = by block size, 0 / 1 / 2 = 64 x 8 / 70 x 7 / 54 x 9 threads
   unsigned only_mask = 0xffffffffu;  // cfd_profile_only: kernel classes (bit = ProfClass id) that launch_rhs still launches
   int xi_mode = 0;                    // xi kernel (cfd_set_sweep_plan): 0 chunk ring + 16-byte cp.async, 1 (plan 5) chunk ring + TMA, 2 (plan 4) 8-byte cp.async staging
   std::string err;

@@ -262,10 +262,14 @@ __global__ void __launch_bounds__(G::NT, G::MINB) k_visc_march(const __grid_cons
 }
 
 using G0 = VG<64, 8>;
+using G1 = VG<70, 7>;
+using G2 = VG<54, 9>;
 
 }  // namespace
 
 int visc_march_init() {
+  if (cudaFuncSetAttribute(k_visc_march<G1>, cudaFuncAttributeMaxDynamicSharedMemorySize, G1::SMEM) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(k_visc_march<G2>, cudaFuncAttributeMaxDynamicSharedMemorySize, G2::SMEM) != cudaSuccess) return -1;
   return cudaFuncSetAttribute(k_visc_march<G0>, cudaFuncAttributeMaxDynamicSharedMemorySize, G0::SMEM) == cudaSuccess ? 0 : -1;
 }
 
@@ -273,8 +277,30 @@ int visc_march_init() {
 // Tile geometry: 64 x 8 threads.  Measured on B200 (256^3, 128^3, 8 x 96^3): 70 x 7 (12 % fewer thread-planes at 256^3),
 // 54 x 9 and two 64 x 4 CTAs per SM all land within +-5 % of it -- the kernel is bound by the shared-memory pipe and the
 // per-plane barrier, not by the tile's halo overhead -- so only this one is instantiated.
+template <class G>
+static long long visc_thread_planes(const BlockDev& B) {
+  const int TImax = G::VX - 6;
+  const long long ntile = (B.n[0] + TImax - 1) / TImax, rows = (B.n[1] + 6 + G::VY - 1) / G::VY;
+  return ntile * rows * G::NT;
+}
+template <class G>
+static int launch_visc_march_g(cfd_ctx* c, const BlockDev& B);
+
+// Tile geometry: the one with the fewest thread-planes for this block (64 x 8, 70 x 7 or 54 x 9 threads: 58, 64 or 48
+// output columns per tile row; measured at 256^3: 1.005 / 1.031 / 1.103 ms, at 128^3: 0.166 / 0.180 / 0.159 ms);
+// cfd_set_visc_tile forces one (tests, measurements).
 int launch_visc_march(cfd_ctx* c, const BlockDev& B) {
-  using G = G0;
+  const int force = c->visc_tile;
+  const long long t0 = visc_thread_planes<G0>(B), t1 = visc_thread_planes<G1>(B), t2 = visc_thread_planes<G2>(B);
+  int g = 0;
+  if (t1 < t0 && t1 <= t2) g = 1;
+  else if (t2 < t0 && t2 < t1) g = 2;
+  if (force >= 0) g = force;
+  return g == 1 ? launch_visc_march_g<G1>(c, B) : (g == 2 ? launch_visc_march_g<G2>(c, B) : launch_visc_march_g<G0>(c, B));
+}
+
+template <class G>
+static int launch_visc_march_g(cfd_ctx* c, const BlockDev& B) {
   if (B.M + 2 >= (1LL << 32)) { c->err = "k_visc_march: block too large for 32-bit element offsets"; return CFD_E_ARG; }
   const int TImax = G::VX - 6;
   const int ntile = (B.n[0] + TImax - 1) / TImax;

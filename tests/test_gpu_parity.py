@@ -632,3 +632,18 @@ def test_profile_only_masks_kernel_classes_and_default_restores_parity(po, W, B)
     assert float(g.interior(0, "r").abs().max()) != 7.0
     g.profile_only()                # default: all classes, and the RHS meets the oracle again
     assert_rhs_parity(o, g, case)
+
+
+@pytest.mark.parametrize("tile", [0, 1, 2])
+def test_visc_tile_geometries_agree_bit_for_bit_and_meet_the_oracle(po, W, B, tile):
+    """cfd_set_visc_tile: the three tile geometries of k_visc_march (64 x 8, 70 x 7, 54 x 9 threads) on a ragged block that
+    spans several tiles of each: the cylinder recipe (wall + far field) at 150 x 21 x 17."""
+    case = W.c5_cylinder(ni=150, nj=21, nk=17)
+    o, g = pair(po, B, case)
+    g.set_visc_tile(tile)
+    assert_rhs_parity(o, g, case)
+    r_t = g.to_numpy(0, "r").copy()
+    g.set_visc_tile(0)
+    g.rhs()
+    assert np.array_equal(g.to_numpy(0, "r"), r_t)
+    g.set_visc_tile(-1)
