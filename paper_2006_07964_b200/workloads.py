@@ -338,6 +338,35 @@ def c5_cylinder(ni=1024, nj=256, nk=128, ratio=1.02, r_out=20.0, steps=50, seed=
                 dt=0.5 * hmin / (1.0 + mach) / 1.8, steps=steps, meta=dict(dr0=dr0, hmin=hmin))
 
 
+def c5_cylinder_split(nblk=2, **kw):
+    """The cylinder of c5_cylinder cut along the azimuth into nblk point-matched blocks (INTERFACE faces in xi, also across
+    theta = 0; WALL / FARFIELD in eta and the periodic span in zeta on every block): physical boundary conditions next to
+    block interfaces, the case the paper's bc_block + bc_phys order is for (Fig. 2).  Same nodes and field as
+    the single block, so the two runs must agree point for point."""
+    one = c5_cylinder(**kw)
+    ni, nj, nk = one.dims[0]
+    if ni % nblk or ni // nblk < 6:
+        raise ValueError("c5_cylinder_split: ni must be a multiple of nblk with at least 6 nodes per block")
+    nb = ni // nblk
+    Lz = np.pi
+    dims, xyz, q0, faces = [], [], [], []
+    for b in range(nblk):
+        sl = slice(b * nb, (b + 1) * nb)
+        dims.append((nb, nj, nk))
+        xyz.append(np.ascontiguousarray(one.xyz[0][..., sl]))
+        q0.append(np.ascontiguousarray(one.q0[0][..., sl]))
+        eye = dict(perm=[0, 1, 2], sign=[1, 1, 1])
+        faces.append(dict(block=b, face=0, type=INTERFACE, nbr_block=(b - 1) % nblk, nbr_face=1, shift=[0.0] * 3, **eye))
+        faces.append(dict(block=b, face=1, type=INTERFACE, nbr_block=(b + 1) % nblk, nbr_face=0, shift=[0.0] * 3, **eye))
+        faces.append(dict(block=b, face=2, type=WALL, nbr_block=-1, nbr_face=-1, shift=[0.0] * 3, **eye))
+        faces.append(dict(block=b, face=3, type=FARFIELD, nbr_block=-1, nbr_face=-1, shift=[0.0] * 3, **eye))
+        for s2 in range(2):
+            faces.append(dict(block=b, face=4 + s2, type=PERIODIC, nbr_block=b, nbr_face=5 - s2,
+                              shift=[0.0, 0.0, -Lz if s2 == 0 else Lz], **eye))
+    return Case(f"C5-cylinder-{nblk}-blocks", dims, xyz, q0, faces, dict(one.params), dt=one.dt, steps=one.steps,
+                meta=dict(one.meta, nblk=nblk, single=one))
+
+
 def sweep_block(n=256, viscous=1, seed=SEED0 + 3, mach=0.1):
     """Throughput sweep block (256^3 / 384^3 / 512^3): C3's mapping and field (SURVEY §8(d) 'Sweep')."""
     c = c3_tgv(n=n, viscous=viscous, steps=20, seed=seed, mach=mach)

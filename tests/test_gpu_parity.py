@@ -647,3 +647,31 @@ def test_visc_tile_geometries_agree_bit_for_bit_and_meet_the_oracle(po, W, B, ti
     g.rhs()
     assert np.array_equal(g.to_numpy(0, "r"), r_t)
     g.set_visc_tile(-1)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Physical BCs next to block interfaces: the cylinder cut along the azimuth (INTERFACE faces beside WALL / FARFIELD)
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nblk", [2, 3])
+def test_split_cylinder_parity_and_equality_with_single_block(po, W, B, nblk):
+    multi = W.c5_cylinder_split(nblk, ni=96, nj=20, nk=10, noise=1e-2)
+    single = multi.meta["single"]
+    om, gm = pair(po, B, multi)
+    assert_rhs_parity(om, gm, multi)
+    g1 = B.Context(single.dims, single.faces, single.params)
+    g1.load_case(single)
+    dt = om.cfl_dt(0.5)
+    for _ in range(4):
+        ro = om.step(dt)
+        rg = gm.step(dt, want_res=True)
+        g1.step(dt)
+    cat = lambda name: np.concatenate([gm.to_numpy(b, name) for b in range(nblk)], axis=-1)
+    qo = np.concatenate([om.interior(b, "q") for b in range(nblk)], axis=-1)
+    assert np.abs(cat("q") - qo).max() < 1e-11 * np.abs(qo).max()
+    assert np.allclose(rg, ro, rtol=1e-10)
+    # the multi-block GPU run equals the single-block GPU run bit for bit (S5 + S6 next to each other)
+    assert np.array_equal(cat("q"), g1.to_numpy(0, "q"))
+    g1.rhs()
+    gm.rhs()
+    assert np.array_equal(cat("r")[:, :, 1:-1], g1.to_numpy(0, "r")[:, :, 1:-1])   # BC-owned node planes excluded (see the oracle test)
+    g1.close()

@@ -389,3 +389,41 @@ def test_create_rejects_bad_topology(po, W):
     bad[0]["nbr_face"] = 3  # axis mismatch with perm
     with pytest.raises(ValueError):
         po.Oracle(case.dims, bad, case.params)
+
+
+# ------------------------------------------------------------------------------------------------
+# Physical boundary conditions NEXT to block interfaces (Fig. 2's bc_block -> bc_phys order; U12-U15):
+# the cylinder cut along the azimuth into point-matched blocks must reproduce the single-block cylinder.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nblk", [2, 3])
+def test_split_cylinder_with_wall_and_far_field_matches_single_block(po, W, nblk):
+    multi = W.c5_cylinder_split(nblk, ni=48, nj=14, nk=8, noise=1e-2)
+    single = multi.meta["single"]
+    o1, om = make(po, single), make(po, multi)
+    nb = multi.dims[0][0]
+    cat = lambda name: np.concatenate([om.interior(b, name) for b in range(nblk)], axis=-1)
+    # metrics: the ghost coordinates behind an interface are the neighbour's nodes, behind wall / far field the same
+    # reflection / extrapolation as in the single block
+    assert np.array_equal(cat("jac"), o1.interior(0, "jac"))
+    assert np.array_equal(cat("khat"), o1.interior(0, "khat"))
+    # R agrees bit for bit on every node the scheme advances.  On the two node planes that the physical BCs own (j = 0 wall,
+    # j = nj-1 far field) R is never used -- the BC overwrites those nodes after every stage -- and there it depends on
+    # ghost cells outside the range the BC refreshes (the viscous reach is +-6 along xi, the BC covers the tangential range
+    # [-3, n+3)): those hold the image of the node plane from BEFORE the BC, whichever block they were copied from.
+    o1.rhs()
+    om.rhs()
+    R1, Rm = o1.interior(0, "r"), cat("r")
+    assert np.array_equal(Rm[:, :, 1:-1], R1[:, :, 1:-1])
+    assert np.abs(Rm - R1).max() < 1e-3 * np.abs(R1).max()
+    dt = o1.cfl_dt(0.5)
+    assert om.cfl_dt(0.5) == dt
+    for _ in range(4):
+        r1 = o1.step(dt)
+        rm = om.step(dt)
+    assert np.array_equal(cat("q"), o1.interior(0, "q"))
+    # U17 sums R^2 over ALL interior nodes, the BC-owned planes included: the residuals agree only as far as those do
+    assert np.allclose(r1, rm, rtol=1e-5)
+    # the wall did something: the velocity at the wall nodes is zero, away from it not
+    q = cat("q")
+    assert np.abs(q[1:4, :, 0, :]).max() == 0.0 and np.abs(q[1, :, 3, :]).max() > 0.05
+    assert nb * nblk == 48

@@ -248,3 +248,45 @@ def test_bench_sharded_line_on_one_gpu():
     assert d["scaling"] == "strong" and d["n_gpus"] == 1 and d["unit"] == "Gpts/s"
     assert d["config"]["owner"] == [0] * 8 and d["config"]["halo_bytes_pulled_per_stage_rank0"] == 0
     assert d["state_finite"] and d["value"] > 0.5 and d["e2e"]["value"] > 0 and d["gpu_launches"] > 0
+
+
+@pytest.mark.gpu
+def test_sharded_contexts_with_physical_bcs_match_unsharded(W):
+    """The second collective of the sharded stage (between the P2P ghost fill and the BCs): the cylinder cut into four
+    blocks, two per "rank", wall and far field next to remote interfaces."""
+    from paper_2006_07964_b200.sharded import ShardedContext, partition_blocks
+
+    case = W.c5_cylinder_split(4, ni=96, nj=20, nk=10, noise=1e-2)
+    q1, _, res1, dt1 = _single(case, 2)
+    owner = partition_blocks(case.dims, 2)
+
+    class FakeComm:
+        def __init__(self, r):
+            self.rank, self.world = r, 2
+
+    ctxs = [ShardedContext(case.dims, case.faces, case.params, owner, FakeComm(r), device="cuda:0", defer_create=True) for r in range(2)]
+    assert all(c.has_bc for c in ctxs)
+    for c in ctxs:
+        o = ctxs[1 - c.rank]
+        c.create(peer_fields={b: {n: o.fields[b][n] for n in ("q", "qn", "r", "xyz")} for b in o.local})
+        c.comm = None
+    for c in ctxs:
+        c.load_local(case)
+    for phase in range(3):
+        for c in ctxs:
+            c.finish_load(phase)
+    for _ in range(2):
+        for s in (1, 2, 3):
+            parts = [c.stage_local(s, case.dt, want_res=(s == 1)) for c in ctxs]
+            for c in ctxs:
+                c.exchange()
+            for c in ctxs:
+                c.apply_bc()
+            if s == 1:
+                res = np.sum(parts, axis=0)
+    for c in ctxs:
+        for b in c.local:
+            assert np.array_equal(c.interior(b, "q").cpu().numpy(), q1[b]), f"block {b}"
+    assert np.allclose(res, res1, rtol=1e-13, atol=0.0)
+    for c in ctxs:
+        c.close()
