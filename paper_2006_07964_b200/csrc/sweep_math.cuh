@@ -22,15 +22,18 @@ __device__ __forceinline__ void weno_corr(double D1, double D2, double D3, doubl
   const double dB = fma((13.0 / 3.0) * t3, t3, fma(t4, t4, eps4));
   const double dC = fma((13.0 / 3.0) * t5, t5, fma(t6, t6, eps4));
   const double pA = dB * dC, pB = dA * dC, pC = dA * dB;
-  const double sA = pA * pA, sB = (10.0 * pB) * pB, sC = pC * pC;  // 16 gamma_k alpha_k (dA dB dC)^2
+  const double sA = pA * pA, sC = pC * pC, pB10 = 10.0 * pB;  // 16 gamma_k alpha_k (dA dB dC)^2; sB = pB10 pB only inside the sums
   const double g1 = t1 - t3, g2 = t5 - t3;
   const double x = sA * g1, y = sC * g2;
-  const double denL = fma(5.0, sC, sA + sB), denR = fma(5.0, sA, sB + sC);
+  const double denL = fma(pB10, pB, fma(5.0, sC, sA)), denR = fma(pB10, pB, fma(5.0, sA, sC));
   const double numL = fma(0.375, x, -0.625 * y), numR = fma(0.375, y, -0.625 * x);
   const double inv = frcp(denL * denR);
   cL = (numL * denR) * inv;
   cR = (numR * denL) * inv;
 }
+
+__device__ __forceinline__ double pos_part(double x) { return __double2hiint(x) < 0 ? 0.0 : x; }   // max(x, 0)
+__device__ __forceinline__ double neg_part(double x) { return __double2hiint(x) < 0 ? x : 0.0; }   // min(x, 0)
 
 // Steger–Warming split flux (U3) of state U through the interface metric (kx,ky,kz), kn = |k|, ikn = 1/|k|.
 template <int SGN>
@@ -46,17 +49,20 @@ __device__ __forceinline__ void sw_flux(const double U[5], double kx, double ky,
   const double th = fma(kx, u, fma(ky, v, kz * w));
   const double ck = c * kn;
   double l1 = th, l4 = th + ck, l5 = th - ck;
-  if (SGN > 0) { l1 = fmax(l1, 0.0); l4 = fmax(l4, 0.0); l5 = fmax(l5, 0.0); }  // (l + |l|)/2 exactly
-  else { l1 = fmin(l1, 0.0); l4 = fmin(l4, 0.0); l5 = fmin(l5, 0.0); }
+  // (l +- |l|)/2 exactly = max / min(l, 0); decided on the sign bit with integer instructions (a DSETP would take an
+  // FP64-pipe slot, and that pipe is what bounds the sweeps)
+  if (SGN > 0) { l1 = pos_part(l1); l4 = pos_part(l4); l5 = pos_part(l5); }
+  else { l1 = neg_part(l1); l4 = neg_part(l4); l5 = neg_part(l5); }
   const double a1 = (2.0 * g1) * l1, s45 = l4 + l5, d45 = l4 - l5;
   const double f = U[0] * (0.5 / gamma);
-  const double fA = f * (a1 + s45), fc = f * ((c * ikn) * d45);
+  const double fs = f * s45;
+  const double fA = fma(f, a1, fs), fc = f * ((c * ikn) * d45);
   F[0] = fA;
   F[1] = fma(fA, u, fc * kx);
   F[2] = fma(fA, v, fc * ky);
   F[3] = fma(fA, w, fc * kz);
   // 0.5 a1 q2 + 0.5 s45 (q2 + c2) + cn th + (3-g)/(2(g-1)) s45 c2  =  q2/2 (a1+s45) + cn th + s45 c2/(g-1)
-  F[4] = fma(0.5 * q2, fA, fma(fc, th, ((f * s45) * c2) * (1.0 / g1)));
+  F[4] = fma(0.5 * q2, fA, fma(fc, th, (fs * c2) * (1.0 / g1)));
 }
 
 // U5: symmetric 6-point Lagrange (150, -25, 3)/256
@@ -111,15 +117,15 @@ __device__ __forceinline__ void afweno_states(const double Qs[5][5], double kx, 
     const double d0 = Qs[s + 1][0] - Qs[s][0], d1 = Qs[s + 1][1] - Qs[s][1], d2 = Qs[s + 1][2] - Qs[s][2],
                  d3 = Qs[s + 1][3] - Qs[s][3], d4 = Qs[s + 1][4] - Qs[s][4];
     const double dx = fma(-d0, u, d1), dy = fma(-d0, v, d2), dz = fma(-d0, w, d3);
-    const double E = fma(hq, d0, d4) - fma(u, d1, fma(v, d2, w * d3));
+    const double E = fma(-w, d3, fma(-v, d2, fma(-u, d1, fma(hq, d0, d4))));
     const double A = fma(-b1, E, d0);
     const double nd = fma(nx, dx, fma(ny, dy, nz * dz));
     V[0][s] = fma(nx, A, fma(nz, dy, -ny * dz));
     V[1][s] = fma(ny, A, fma(nx, dz, -nz * dx));
     V[2][s] = fma(nz, A, fma(ny, dx, -nx * dy));
-    const double x = hg * E, y = hc * nd;  // (g-1) E / (2 c^2),  c n.dm / (2 c^2)
-    V[3][s] = x + y;
-    V[4][s] = x - y;
+    const double y = hc * nd;  // c n.dm / (2 c^2);  hg E = (g-1) E / (2 c^2)
+    V[3][s] = fma(hg, E, y);
+    V[4][s] = fma(hg, E, -y);
   }
   double cL[5], cR[5];
 #pragma unroll
@@ -156,9 +162,9 @@ __device__ __forceinline__ double weno_corr_left(double D1, double D2, double D3
   const double dB = fma((13.0 / 3.0) * t3, t3, fma(t4, t4, eps4));
   const double dC = fma((13.0 / 3.0) * t5, t5, fma(t6, t6, eps4));
   const double pA = dB * dC, pB = dA * dC, pC = dA * dB;
-  const double sA = pA * pA, sB = (10.0 * pB) * pB, sC = pC * pC;
+  const double sA = pA * pA, sC = pC * pC;
   const double x = sA * (t1 - t3), y = sC * (t5 - t3);
-  return fma(0.375, x, -0.625 * y) * frcp(fma(5.0, sC, sA + sB));
+  return fma(0.375, x, -0.625 * y) * frcp(fma(10.0 * pB, pB, fma(5.0, sC, sA)));
 }
 __device__ __forceinline__ double weno_corr_right(double D1, double D2, double D3, double D4, double eps4) {
   const double t1 = D2 - D1, t3 = D3 - D2, t5 = D4 - D3;
@@ -167,9 +173,9 @@ __device__ __forceinline__ double weno_corr_right(double D1, double D2, double D
   const double dB = fma((13.0 / 3.0) * t3, t3, fma(t4, t4, eps4));
   const double dC = fma((13.0 / 3.0) * t5, t5, fma(t6, t6, eps4));
   const double pA = dB * dC, pB = dA * dC, pC = dA * dB;
-  const double sA = pA * pA, sB = (10.0 * pB) * pB, sC = pC * pC;
+  const double sA = pA * pA, sC = pC * pC;
   const double x = sA * (t1 - t3), y = sC * (t5 - t3);
-  return fma(0.375, y, -0.625 * x) * frcp(fma(5.0, sA, sB + sC));
+  return fma(0.375, y, -0.625 * x) * frcp(fma(10.0 * pB, pB, fma(5.0, sA, sC)));
 }
 
 __device__ __forceinline__ void afweno_iface_orig(const double Q6[6][5], double kx, double ky, double kz, double ikn, double gamma,
@@ -199,15 +205,15 @@ __device__ __forceinline__ void afweno_iface_orig(const double Q6[6][5], double 
     const double d0 = Q6[s + 1][0] - Q6[s][0], d1 = Q6[s + 1][1] - Q6[s][1], d2 = Q6[s + 1][2] - Q6[s][2],
                  d3 = Q6[s + 1][3] - Q6[s][3], d4 = Q6[s + 1][4] - Q6[s][4];
     const double dx = fma(-d0, u, d1), dy = fma(-d0, v, d2), dz = fma(-d0, w, d3);
-    const double E = fma(hq, d0, d4) - fma(u, d1, fma(v, d2, w * d3));
+    const double E = fma(-w, d3, fma(-v, d2, fma(-u, d1, fma(hq, d0, d4))));
     const double A = fma(-b1, E, d0);
     const double nd = fma(nx, dx, fma(ny, dy, nz * dz));
     V[0][s] = fma(nx, A, fma(nz, dy, -ny * dz));
     V[1][s] = fma(ny, A, fma(nx, dz, -nz * dx));
     V[2][s] = fma(nz, A, fma(ny, dx, -nx * dy));
-    const double x = hg * E, y = hc * nd;
-    V[3][s] = x + y;
-    V[4][s] = x - y;
+    const double y = hc * nd;
+    V[3][s] = fma(hg, E, y);
+    V[4][s] = fma(hg, E, -y);
   }
   double cL[5], cR[5];
 #pragma unroll
