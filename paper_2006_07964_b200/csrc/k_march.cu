@@ -192,10 +192,12 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
         const double kz = khalf(k0[7 * MT], k1[7 * MT], k2[7 * MT], sc[7 * MT], k4[7 * MT], k5[7 * MT]);
         const double kk = fma(kx, kx, fma(ky, ky, kz * kz));
         const double ikn = frsqrt(kk), kn = kk * ikn;
-        double Fp[5], Fm[5];
+        double Ph[5];   // Phi_{j-1/2} = G + F+ + F-: the split fluxes are accumulated onto the FIR output
+#pragma unroll
+        for (int m = 0; m < 5; ++m) Ph[m] = G[m];
         if (SCH == 0) {
-          sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
-          sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+          sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Ph);
+          sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Ph);
         } else {
           double Q6[6][5];
 #pragma unroll
@@ -205,15 +207,15 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
             for (int s = 0; s < 5; ++s) Q6[s + 1][m] = Qs[s][m];
           }
           afweno_iface_orig(Q6, kx, ky, kz, ikn, gamma, eps4, UL, UR);
-          sw_flux<+1>(UL, kx, ky, kz, kn, ikn, gamma, Fp);
-          sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+          sw_flux<+1>(UL, kx, ky, kz, kn, ikn, gamma, Ph);
+          sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Ph);
         }
         const double* so = ocol + ((j - 1) & 1) * (NOUT * MT);
         double jac = 0.0;
         if (ACC >= 2 && j > p0) jac = so[OC::O_J * MT];
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
-          const double Phi = (Fp[m] + Fm[m]) + G[m];
+          const double Phi = Ph[m];
           if (j > p0) {
             const double X = Phip[m] - Phi;
             double* rp = r + m * M + (long long)(j - 1) * sm;
@@ -415,13 +417,15 @@ __global__ void __launch_bounds__(32 * XWARPS, 2) k_march_xi(XiArgs A) {
       const double kz = khalf(sl0[7 * XR], sl1[7 * XR], sl2[7 * XR], sl3[7 * XR], sl4[7 * XR], sl5[7 * XR]);
       const double kk = fma(kx, kx, fma(ky, ky, kz * kz));
       const double ikn = frsqrt(kk), kn = kk * ikn;
-      double Fp[5], Fm[5];
-      sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Fp);
-      sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Fm);
+      double Ph[5];
+#pragma unroll
+      for (int m = 0; m < 5; ++m) Ph[m] = G[m];
+      sw_flux<+1>(ULc, kx, ky, kz, kn, ikn, gamma, Ph);
+      sw_flux<-1>(UR, kx, ky, kz, kn, ikn, gamma, Ph);
       double* park = my + s0;  // Q slots of position j-3
 #pragma unroll
       for (int m = 0; m < 5; ++m) {
-        const double Phi = (Fp[m] + Fm[m]) + G[m];
+        const double Phi = Ph[m];
         if (j > p0) park[m * XR] = Phip[m] - Phi;
         Phip[m] = Phi;
       }

@@ -137,10 +137,12 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
     }
     const double kk = fma(kh[0], kh[0], fma(kh[1], kh[1], kh[2] * kh[2]));
     const double ikn = frsqrt(kk), kn = kk * ikn;
-    double Fp[5], Fm[5];
+    double Ph[5];   // Phi_{j-1/2} = G + F+ + F-: the split fluxes are accumulated onto the FIR output
+#pragma unroll
+    for (int m = 0; m < 5; ++m) Ph[m] = G[m];
     if (SCH == 0) {
-      sw_flux<+1>(st.ULc, kh[0], kh[1], kh[2], kn, ikn, gamma, Fp);
-      sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Fm);
+      sw_flux<+1>(st.ULc, kh[0], kh[1], kh[2], kn, ikn, gamma, Ph);
+      sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Ph);
     } else {
       double Q6[6][5];
 #pragma unroll
@@ -150,12 +152,12 @@ __device__ __forceinline__ void xi_step(XiState& st, char* P0, const char* P1, c
         for (int t = 0; t < 5; ++t) Q6[t + 1][m] = Qs[t][m];
       }
       afweno_iface_orig(Q6, kh[0], kh[1], kh[2], ikn, gamma, eps4, UL, UR);
-      sw_flux<+1>(UL, kh[0], kh[1], kh[2], kn, ikn, gamma, Fp);
-      sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Fm);
+      sw_flux<+1>(UL, kh[0], kh[1], kh[2], kn, ikn, gamma, Ph);
+      sw_flux<-1>(UR, kh[0], kh[1], kh[2], kn, ikn, gamma, Ph);
     }
 #pragma unroll
     for (int m = 0; m < 5; ++m) {
-      const double Phi = (Fp[m] + Fm[m]) + G[m];
+      const double Phi = Ph[m];
       if (store) park[m * pstr] = st.Phip[m] - Phi;
       st.Phip[m] = Phi;
     }

@@ -35,7 +35,7 @@ __device__ __forceinline__ void weno_corr(double D1, double D2, double D3, doubl
 __device__ __forceinline__ double pos_part(double x) { return __double2hiint(x) < 0 ? 0.0 : x; }   // max(x, 0)
 __device__ __forceinline__ double neg_part(double x) { return __double2hiint(x) < 0 ? x : 0.0; }   // min(x, 0)
 
-// Steger–Warming split flux (U3) of state U through the interface metric (kx,ky,kz), kn = |k|, ikn = 1/|k|.
+// Steger–Warming split flux (U3) of state U through the interface metric (kx,ky,kz), kn = |k|, ikn = 1/|k|, ADDED to F.
 template <int SGN>
 __device__ __forceinline__ void sw_flux(const double U[5], double kx, double ky, double kz, double kn, double ikn,
                                         double gamma, double F[5]) {
@@ -57,12 +57,14 @@ __device__ __forceinline__ void sw_flux(const double U[5], double kx, double ky,
   const double f = U[0] * (0.5 / gamma);
   const double fs = f * s45;
   const double fA = fma(f, a1, fs), fc = f * ((c * ikn) * d45);
-  F[0] = fA;
-  F[1] = fma(fA, u, fc * kx);
-  F[2] = fma(fA, v, fc * ky);
-  F[3] = fma(fA, w, fc * kz);
+  // F is IN/OUT: the split flux is ADDED to what F holds (the caller seeds it with the central part of Phi and chains the
+  // two split fluxes), so that the sums Phi = F+ + F- + G ride in the FMAs of the flux rows instead of separate DADDs
+  F[0] += fA;
+  F[1] = fma(fA, u, fma(fc, kx, F[1]));
+  F[2] = fma(fA, v, fma(fc, ky, F[2]));
+  F[3] = fma(fA, w, fma(fc, kz, F[3]));
   // 0.5 a1 q2 + 0.5 s45 (q2 + c2) + cn th + (3-g)/(2(g-1)) s45 c2  =  q2/2 (a1+s45) + cn th + s45 c2/(g-1)
-  F[4] = fma(0.5 * q2, fA, fma(fc, th, (fs * c2) * (1.0 / g1)));
+  F[4] = fma(0.5 * q2, fA, fma(fc, th, fma(fs * c2, 1.0 / g1, F[4])));
 }
 
 // U5: symmetric 6-point Lagrange (150, -25, 3)/256
