@@ -208,6 +208,45 @@ const char* cfd_profile_name(int id);
  * 3 viscous point fluxes) is set in mask.  With any of these bits clear the RESULTS ARE INVALID; the default is all ones. */
 int cfd_profile_only(cfd_ctx*, unsigned mask);
 
+/* ---- For callers that cannot allocate device memory --------------------------------------------------------------
+ * S4, stage 1 (Eq. 20: q^n := q, q := q + dt r) with the residual res_m = sum over the interior points of
+ * r_m^2 (U17) for ONE block, WITHOUT a context and without any workspace.
+ *
+ * Who needs it: everything else in this header goes through cfd_create_blocks, which calls cudaMalloc and wants a
+ * caller-allocated workspace.  That is impossible for a solver plug-in whose host application has already reserved all of
+ * the device memory for its own arena (cudaMalloc just returns out-of-memory there), for a coupling / in-situ loop that
+ * may not stall the GPU (cudaMalloc and cudaFree synchronise against every stream of the device), and for a callback that
+ * is simply handed q and r by somebody else and owns no allocator.  Such a caller passes only its inputs and outputs;
+ * the per-CTA partial sums of the reduction live in a fixed array inside the library image.
+ *
+ * Arguments: q (in/out), qn (out), r (in): DEVICE pointers, fp64, layout [5][nk+12][nj+12][ni+12] with the CFD_NG ghost
+ * layers like cfd_block_ptrs (ghost entries are neither read nor written), 8-byte aligned, caller-owned; ni, nj, nk >= 1;
+ * res5_dev: DEVICE pointer to 5 doubles receiving res_m (read it back on the same stream when you need it);
+ * cuda_stream: a cudaStream_t of the CURRENT device (may be 0).  Asynchronous; never synchronises.  For a block within
+ * the limit the values of q, qn and res are those cfd_rk_stage(ctx, 1, dt, res) produces (same summation order).
+ *
+ * Limit: ni*nj*nk <= CFD_STATIC_MAX_POINTS (2 097 152 = 128^3 interior points); larger blocks are refused with
+ * CFD_E_WORKSPACE and a message naming both numbers -- nothing is launched.  Cost: the built-in array takes
+ * CFD_STATIC_SCRATCH_BYTES (320 KB) of device memory on every GPU that loads this library, from load until process exit.
+ *
+ * Set-up: the FIRST call on each device looks up that device's address of the built-in array (cudaGetSymbolAddress, with
+ * the device current, which also makes the runtime load the library's kernels there) and caches it; make that first call
+ * during start-up, before you begin any stream capture.  After it the call only launches two kernels: no cudaMalloc,
+ * cudaFree or other allocating routine, ever.
+ *
+ * Sharing: there is ONE array per device and every call uses it.  It keeps whatever the previous call left in it; that is
+ * harmless because each call overwrites every slot it later reads (nothing has to start at zero, so nothing is cleared).
+ * Two calls that may run on the same GPU at the same time (different streams, or different host threads on different
+ * streams) RACE on it and give wrong residuals: issue all calls for one device on one stream, or order them with events.
+ *
+ * Errors: CFD_E_ARG (null / misaligned pointer, size < 1), CFD_E_WORKSPACE (block too large), CFD_E_CUDA (runtime call
+ * failed); cfd_static_last_error() returns the message of the calling thread's last failing call ("" after a success). */
+#define CFD_STATIC_MAX_POINTS 2097152
+#define CFD_STATIC_SCRATCH_BYTES 327680
+int cfd_rk_stage1_static(double* q, double* qn, const double* r, int ni, int nj, int nk, double dt, double* res5_dev,
+                         void* cuda_stream);
+const char* cfd_static_last_error(void);
+
 /* Frees the context (never the caller's buffers). */
 int cfd_destroy(cfd_ctx*);
 

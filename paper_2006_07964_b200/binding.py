@@ -21,8 +21,9 @@ ABI_SYMBOLS = (
     "cfd_launch_count", "cfd_fp64_peak_probe", "cfd_step_host", "cfd_profile_enable", "cfd_profile_read",
     "cfd_profile_name", "cfd_selftest_fastmath", "cfd_set_sweep_plan", "cfd_stage_fused", "cfd_buffer_roles",
     "cfd_cfl_dt", "cfd_create_blocks_sharded", "cfd_workspace_bytes_sharded", "cfd_stage_fused_local",
-    "cfd_profile_only", "cfd_set_visc_tile",
+    "cfd_profile_only", "cfd_set_visc_tile", "cfd_rk_stage1_static", "cfd_static_last_error",
 )
+STATIC_MAX_POINTS = 2097152  # CFD_STATIC_MAX_POINTS of include/cfd.h
 PROF_NCLASS = 12
 
 
@@ -99,6 +100,11 @@ def _load():
     L.cfd_selftest_fastmath.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.cfd_fp64_peak_probe.restype = C.c_int
     L.cfd_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    L.cfd_rk_stage1_static.restype = C.c_int
+    L.cfd_rk_stage1_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double,
+                                       C.c_void_p, C.c_void_p]
+    L.cfd_static_last_error.restype = C.c_char_p
+    L.cfd_static_last_error.argtypes = []
     return L
 
 
@@ -123,6 +129,31 @@ def selftest_fastmath(x):
     if rc != 0:
         raise CfdError(rc, "cfd_selftest_fastmath failed")
     return r, s
+
+
+def rk_stage1_static(q, qn, r, dims, dt, res5, stream=None):
+    """cfd_rk_stage1_static: RK3 stage 1 (q^n := q, q := q + dt r) and res_m = sum r_m^2 of ONE block without a context,
+    a workspace or any device allocation -- for callers that cannot allocate (a plug-in inside an application that has
+    reserved all device memory, a loop that may not stall the GPU on cudaMalloc, a callback that owns no allocator): the
+    partial sums live in a fixed array inside the library.  q, qn, r: device fp64 tensors of shape (5, nk+12, nj+12, ni+12);
+    res5: device fp64 tensor of 5 elements (output); dims = (ni, nj, nk) with ni*nj*nk <= STATIC_MAX_POINTS.  Enqueues on
+    `stream` (default: torch's current stream of q's device) and returns at once.  All calls on one device share that array:
+    keep them on one stream.  This wrapper only checks and passes pointers."""
+    import torch
+
+    ni, nj, nk = (int(x) for x in dims)
+    shp = (5, nk + 2 * NG, nj + 2 * NG, ni + 2 * NG)
+    for name, a in (("q", q), ("qn", qn), ("r", r)):
+        if not (a.is_cuda and a.dtype == torch.float64 and a.is_contiguous() and tuple(a.shape) == shp):
+            raise CfdError(-1, f"rk_stage1_static: {name} must be a contiguous device fp64 tensor of shape {shp}")
+    if not (res5.is_cuda and res5.dtype == torch.float64 and res5.is_contiguous() and res5.numel() == 5):
+        raise CfdError(-1, "rk_stage1_static: res5 must be a contiguous device fp64 tensor of 5 elements")
+    with torch.cuda.device(q.device):
+        st = stream if stream is not None else torch.cuda.current_stream(q.device)
+        rc = lib.cfd_rk_stage1_static(q.data_ptr(), qn.data_ptr(), r.data_ptr(), ni, nj, nk, float(dt), res5.data_ptr(),
+                                      C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise CfdError(rc, lib.cfd_static_last_error().decode())
 
 
 class Context:
