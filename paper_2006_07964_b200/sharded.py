@@ -206,7 +206,8 @@ class ShardedContext:
 
     def close(self):
         if getattr(self, "h", None):
-            self.B.lib.cfd_destroy(self.h)
+            with self.torch.cuda.device(self.device):
+                self.B.lib.cfd_destroy(self.h)
             self.h = None
 
     def __del__(self):
@@ -218,6 +219,12 @@ class ShardedContext:
     def _chk(self, rc):
         if rc != 0:
             raise self.B.CfdError(rc, self.B.lib.cfd_last_error(self.h).decode())
+
+    def _call(self, fn, *args):
+        """A library call that enqueues work: made with THIS context's device current (its stream and buffers belong to
+        self.device; the process-wide current device may be another one, e.g. with several contexts in one process)."""
+        with self.torch.cuda.device(self.device):
+            self._chk(fn(self.h, *args))
 
     def _barrier(self):
         if self.comm is not None:
@@ -249,11 +256,11 @@ class ShardedContext:
         the phases of all their contexts in turn; `load_case` does it with the communicator)."""
         lib = self.B.lib
         if phase == 0:
-            self._chk(lib.cfd_compute_metrics(self.h))     # pulls the peers' xyz interiors
+            self._call(lib.cfd_compute_metrics)     # pulls the peers' xyz interiors
         elif phase == 1:
-            self._chk(lib.cfd_exchange_interfaces(self.h))  # pulls the peers' q interiors
+            self._call(lib.cfd_exchange_interfaces)  # pulls the peers' q interiors
         else:
-            self._chk(lib.cfd_apply_bc(self.h))
+            self._call(lib.cfd_apply_bc)
 
     def load_case(self, case):
         self.load_local(case)
@@ -265,14 +272,14 @@ class ShardedContext:
     # ---- the sharded stage ----
     def stage_local(self, stage, dt, want_res=False):
         res = (C.c_double * 5)()
-        self._chk(self.B.lib.cfd_stage_fused_local(self.h, int(stage), float(dt), res if want_res else None))
+        self._call(self.B.lib.cfd_stage_fused_local, int(stage), float(dt), res if want_res else None)
         return np.array(res[:]) if want_res else None
 
     def exchange(self):
-        self._chk(self.B.lib.cfd_exchange_interfaces(self.h))
+        self._call(self.B.lib.cfd_exchange_interfaces)
 
     def apply_bc(self):
-        self._chk(self.B.lib.cfd_apply_bc(self.h))
+        self._call(self.B.lib.cfd_apply_bc)
 
     def stage(self, stage, dt, want_res=False):
         """cfd_stage_fused over all ranks: local sweeps + RK, collective, P2P ghost fill, BCs; the stage-1 residual
@@ -316,7 +323,7 @@ class ShardedContext:
     def cfl_dt(self, cfl):
         """min over the ranks of the local cfd_cfl_dt."""
         dt = C.c_double()
-        self._chk(self.B.lib.cfd_cfl_dt(self.h, float(cfl), C.byref(dt), None))
+        self._call(self.B.lib.cfd_cfl_dt, float(cfl), C.byref(dt), None)
         if self.comm is None:
             return dt.value
         return float(self.comm.allreduce([dt.value], "min", self.stream)[0])
