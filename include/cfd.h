@@ -116,8 +116,13 @@ int cfd_create_blocks(cfd_ctx** out, int nblocks, const cfd_dims* dims, const cf
  * cfd_exchange_interfaces (and the xyz fill of cfd_compute_metrics) pull the ghost layers of the local blocks straight
  * out of the owner's interior cells with P2P loads through the same composed index maps -- no packing, no staging
  * buffer, no host copy (on NVSwitch every peer is equidistant, so the paper's topology-aware placement, P:L356–390,
- * has nothing left to decide).  Everything else (metrics, RHS, RK stage, BCs, CFL, step_host) runs on the local blocks
+ * has nothing left to decide).  Everything else (metrics, RHS, RK stage, BCs, CFL) runs on the local blocks
  * only; res5 and the CFL maximum are LOCAL sums / maxima: the caller reduces them over the processes.
+ * The single-call stages cfd_stage, cfd_stage_fused and cfd_step_host are REFUSED (CFD_E_ARG, nothing enqueued) on a
+ * context that has peer-owned blocks: they would run the P2P ghost fill right behind the local sweeps, with no way to
+ * know that the peers have finished writing (or have rotated their buffer roles) -- a silent data race.  Use
+ * cfd_stage_fused_local -> cross-process barrier -> cfd_exchange_interfaces -> barrier -> cfd_apply_bc instead
+ * (paper_2006_07964_b200/sharded.py does).
  * Ordering is the caller's job (the binding does it with collectives on the compute stream): every process must have
  * finished the stage's last sweep before any process runs cfd_exchange_interfaces of that stage, all processes must call
  * the stage functions in lock step (the buffer roles of cfd_stage_fused rotate identically everywhere), and the
@@ -160,7 +165,9 @@ int cfd_apply_bc(cfd_ctx*);
  * dt_local_dev_or_null: if non-null, one DEVICE pointer per block to a caller-owned array of M doubles (field layout with
  * ghosts); the local time step cfl / s_i is written at interior points (ghost entries untouched).
  * Requires cfd_compute_metrics.  One bandwidth-bound pass over q, khat, jac (120 B per point).
- * Returns host values: synchronises the stream.  CFD_E_ARG if cfl <= 0 or the state is not physical (max s not > 0). */
+ * Returns host values: synchronises the stream.  CFD_E_ARG if cfl <= 0 or the state is not physical: a single interior
+ * point with rho <= 0, p < 0 or a NaN makes s_i NaN, the reduction keeps NaNs (it is not an fmax), and the call fails
+ * instead of returning a dt from the remaining points (dt_local then holds NaN at the offending points). */
 int cfd_cfl_dt(cfd_ctx*, double cfl, double* dt_host, double* const* dt_local_dev_or_null);
 
 /* Convenience: the four calls above for one stage, in Fig. 2's order, on the context's stream. */
@@ -205,7 +212,9 @@ const char* cfd_profile_name(int id);
 
 /* Measurement aid (power / clock measurements of one kernel class looped alone, profiles/r2_power.md): cfd_rhs and
  * cfd_stage_fused launch only the hot kernel classes whose bit (1 << class id: 0 xi sweep, 1 eta sweep, 2 zeta sweep,
- * 3 viscous point fluxes) is set in mask.  With any of these bits clear the RESULTS ARE INVALID; the default is all ones. */
+ * 3 viscous point fluxes) is set in mask.  With any of these bits clear the RESULTS ARE INVALID; the default is all ones.
+ * While such a mask is active every cfd_rhs / cfd_stage_fused[_local] call still returns 0 but leaves "cfd_profile_only mask
+ * active ... INVALID" in cfd_last_error, so that a masked result cannot pass for a valid one; restoring all ones clears it. */
 int cfd_profile_only(cfd_ctx*, unsigned mask);
 
 /* ---- For callers that cannot allocate device memory --------------------------------------------------------------

@@ -384,7 +384,10 @@ extern "C" int cfd_cfl_dt(cfd_ctx* c, double cfl, double* dt_host, double* const
   double smax = 0.0;
   CUDA_TRY(c, cudaMemcpyAsync(&smax, c->d_res + 5, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  if (!(smax > 0.0) || smax != smax) { c->err = "cfd_cfl_dt: non-positive or NaN spectral radius (state not physical)"; return CFD_E_ARG; }
+  if (!(smax > 0.0) || smax != smax || smax > 1.7976931348623157e308) {
+    c->err = "cfd_cfl_dt: non-positive, infinite or NaN spectral radius (state not physical: rho <= 0 or p < 0 at an interior point)";
+    return CFD_E_ARG;
+  }
   *dt_host = cfl / smax;
   return CFD_OK;
 }
@@ -399,8 +402,22 @@ extern "C" int cfd_apply_bc(cfd_ctx* c) {
   return launch_bc_q(c);
 }
 
+// The single-call stages run the ghost fill right behind the local sweeps.  On a context with peer-owned blocks that fill
+// reads the peers' interiors over P2P, and nothing in this process can know whether the peers have finished writing their
+// new state (or have rotated their buffer roles): the caller must put a cross-process barrier in between, which only the
+// split sequence cfd_stage_fused_local -> barrier -> cfd_exchange_interfaces -> barrier -> cfd_apply_bc allows.
+static int refuse_if_sharded(cfd_ctx* c, const char* fn) {
+  if (!c->has_remote()) return CFD_OK;
+  c->err = std::string(fn) + ": this context has blocks owned by peer processes (cfd_create_blocks_sharded); the ghost fill must "
+           "be separated from the sweeps by a cross-process barrier: call cfd_stage_fused_local, synchronise the processes, then "
+           "cfd_exchange_interfaces and cfd_apply_bc";
+  return CFD_E_ARG;
+}
+
 extern "C" int cfd_stage(cfd_ctx* c, int stage, double dt, double* res5) {
   int rc;
+  if (!c) return CFD_E_ARG;
+  if ((rc = refuse_if_sharded(c, "cfd_stage")) != 0) return rc;
   if ((rc = cfd_rhs(c)) != 0) return rc;
   if ((rc = cfd_rk_stage(c, stage, dt, res5)) != 0) return rc;
   if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
@@ -423,7 +440,10 @@ extern "C" int cfd_stage_fused_local(cfd_ctx* c, int stage, double dt, double* r
 }
 
 extern "C" int cfd_stage_fused(cfd_ctx* c, int stage, double dt, double* res5) {
-  int rc = cfd_stage_fused_local(c, stage, dt, res5);
+  if (!c) return CFD_E_ARG;
+  int rc = refuse_if_sharded(c, "cfd_stage_fused");
+  if (rc != 0) return rc;
+  rc = cfd_stage_fused_local(c, stage, dt, res5);
   if (rc != 0) return rc;
   if ((rc = cfd_exchange_interfaces(c)) != 0) return rc;
   return cfd_apply_bc(c);
@@ -437,6 +457,7 @@ extern "C" int cfd_buffer_roles(const cfd_ctx* c, int roles[3]) {
 
 extern "C" int cfd_step_host(cfd_ctx* c, const double* const* qin, double* const* qout, double dt, double* res5) {
   if (!c || !qin || !qout) return CFD_E_ARG;
+  if (int rs = refuse_if_sharded(c, "cfd_step_host")) return rs;
   auto copy3d = [&](const BlockDev& B, double* dev, double* host, bool to_dev) {
     cudaMemcpy3DParms p;
     memset(&p, 0, sizeof(p));
@@ -512,6 +533,7 @@ extern "C" int cfd_set_visc_tile(cfd_ctx* c, int tile) {
 extern "C" int cfd_profile_only(cfd_ctx* c, unsigned mask) {
   if (!c) return CFD_E_ARG;
   c->only_mask = mask;
+  if ((mask & 0xFu) == 0xFu && c->err.rfind("cfd_profile_only mask active", 0) == 0) c->err.clear();  // warning of launch_rhs
   return CFD_OK;
 }
 

@@ -58,6 +58,7 @@ struct cfd_ctx {
   std::vector<BlockDev> blk;
   std::vector<char> local;            // NEXT-4: local[b] = 0 for a block owned by a peer GPU (its pointers are peer-mapped; only the ghost fill reads them)
   bool is_local(size_t b) const { return local.empty() || local[b] != 0; }
+  bool has_remote() const { for (char l : local) if (!l) return true; return false; }  // some block is advanced by a peer process
   std::vector<cfd_face> faces;
   std::vector<CopyTask> tasks[4];     // per pass 1..3
   std::vector<BcTask> bcs;

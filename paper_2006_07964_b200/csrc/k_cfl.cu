@@ -11,6 +11,10 @@ namespace {
 
 constexpr int CT = 256;
 
+// max that KEEPS a NaN (fmax drops it): a point with rho <= 0 or p < 0 gives s = NaN (or Inf), and the reduction must carry
+// that to the host so that cfd_cfl_dt can refuse the state instead of returning a dt from the remaining points.
+__device__ __forceinline__ double max_nan(double a, double b) { return (b > a || b != b) ? b : a; }
+
 __global__ void __launch_bounds__(CT) k_cfl(BlockDev B, double gamma, double cfl, double* __restrict__ partials,
                                             double* __restrict__ dt_local) {
   const int ni = B.n[0], nj = B.n[1];
@@ -34,24 +38,25 @@ __global__ void __launch_bounds__(CT) k_cfl(BlockDev B, double gamma, double cfl
       const double kx = J * B.khat[(d * 3 + 0) * M + p], ky = J * B.khat[(d * 3 + 1) * M + p], kz = J * B.khat[(d * 3 + 2) * M + p];
       s += fabs(kx * u + ky * v + kz * w) + c * sqrt(kx * kx + ky * ky + kz * kz);
     }
+    if (!(rho > 0.0) || !(pr >= 0.0)) s = __longlong_as_double(0x7ff8000000000000LL);  // rho <= 0 with p < 0 would give a real c
     if (dt_local) dt_local[p] = cfl / s;
-    mx = fmax(mx, s);
+    mx = max_nan(mx, s);
   }
   __shared__ double sm[CT / 32];
-  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+  for (int o = 16; o > 0; o >>= 1) mx = max_nan(mx, __shfl_down_sync(0xffffffffu, mx, o));
   if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = mx;
   __syncthreads();
   if (threadIdx.x == 0) {
     double v = sm[0];
-    for (int w = 1; w < CT / 32; ++w) v = fmax(v, sm[w]);
+    for (int w = 1; w < CT / 32; ++w) v = max_nan(v, sm[w]);
     partials[blockIdx.x] = v;
   }
 }
 
 __global__ void k_cfl_final(const double* __restrict__ partials, int n, double* __restrict__ out) {
   double v = 0.0;
-  for (int t = threadIdx.x; t < n; t += 32) v = fmax(v, partials[t]);
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  for (int t = threadIdx.x; t < n; t += 32) v = max_nan(v, partials[t]);
+  for (int o = 16; o > 0; o >>= 1) v = max_nan(v, __shfl_down_sync(0xffffffffu, v, o));
   if (threadIdx.x == 0) *out = v;
 }
 

@@ -87,5 +87,9 @@ int launch_rhs(cfd_ctx* c, int fused_stage, double dt) {
     c->launches++;
   }
   CUDA_TRY(c, cudaGetLastError());
+  // cfd_profile_only: with a hot kernel class masked out the call still returns 0 (the power probe loops it), but the
+  // context says so in cfd_last_error, so that an invalid r / state can never pass for a valid one unnoticed
+  if ((c->only_mask & 0xFu) != 0xFu)
+    c->err = "cfd_profile_only mask active (a hot kernel class is switched off): the results of this call are INVALID";
   return CFD_OK;
 }

@@ -564,6 +564,32 @@ def test_cfl_dt_matches_oracle(po, W, B, which):
         g.cfl_dt(0.0)
 
 
+@pytest.mark.parametrize("bad", ["negative-pressure", "negative-density-and-pressure", "nan"])
+def test_cfl_dt_refuses_a_single_non_physical_point(W, B, bad):
+    """One bad interior point among 32^3 good ones must surface as CFD_E_ARG (include/cfd.h), not be dropped by the MAX
+    reduction: c = sqrt(gamma p / rho) is NaN for p < 0, and real again when rho and p are both negative."""
+    case = W.c1_vortex(32)
+    g = B.Context(case.dims, case.faces, case.params)
+    g.load_case(case)
+    good = g.cfl_dt(0.5)
+    assert good > 0
+    q = g.interior(0, "q")
+    k, j, i = 17, 5, 29  # not in the first thread / first CTA of the reduction
+    if bad == "negative-pressure":
+        q[4, k, j, i] = 0.25 * (q[1, k, j, i] ** 2) / q[0, k, j, i]  # e below the kinetic energy: p < 0
+    elif bad == "negative-density-and-pressure":
+        q[0, k, j, i] = -q[0, k, j, i]
+        q[4, k, j, i] = -q[4, k, j, i]
+    else:
+        q[2, k, j, i] = float("nan")
+    with pytest.raises(B.CfdError) as e:
+        g.cfl_dt(0.5)
+    assert e.value.code == -1 and "not physical" in str(e.value)
+    # the context stays usable once the state is repaired
+    g.interior(0, "q").copy_(__import__("torch").from_numpy(np.ascontiguousarray(case.q0[0])))
+    assert g.cfl_dt(0.5) == good
+
+
 # ------------------------------------------------------------------------------------------------
 # NEXT-3: Sutherland viscosity mu(T) and a shocked workload (shock-vortex slab on the seeded wavy periodic grid)
 # ------------------------------------------------------------------------------------------------
@@ -626,11 +652,14 @@ def test_profile_only_masks_kernel_classes_and_default_restores_parity(po, W, B)
     g.rhs()
     assert g.launch_count == n0
     assert float(g.interior(0, "r").min()) == -7.0 and float(g.interior(0, "r").max()) == -7.0
+    assert "INVALID" in B.lib.cfd_last_error(g.h).decode()   # rc 0, but the context says the result is not one
     g.profile_only(1 << 0)          # the xi sweep alone: one launch, r = X^xi only (not the RHS)
     g.rhs()
     assert g.launch_count == n0 + 1
     assert float(g.interior(0, "r").abs().max()) != 7.0
+    assert "INVALID" in B.lib.cfd_last_error(g.h).decode()
     g.profile_only()                # default: all classes, and the RHS meets the oracle again
+    assert B.lib.cfd_last_error(g.h).decode() == ""
     assert_rhs_parity(o, g, case)
 
 

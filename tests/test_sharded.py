@@ -122,7 +122,10 @@ def _single(case, steps):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("world", [2, 3])
-def test_sharded_contexts_in_one_process_match_unsharded_bit_for_bit(W, world):
+def test_sharded_contexts_in_one_process_match_unsharded_bit_for_bit(W, po, world):
+    import ctypes as C
+
+    from paper_2006_07964_b200 import binding as B
     from paper_2006_07964_b200.sharded import NG, ShardedContext, partition_blocks
 
     case = W.c4_multiblock(nb=12, mach=0.3)
@@ -148,6 +151,18 @@ def test_sharded_contexts_in_one_process_match_unsharded_bit_for_bit(W, world):
     for phase in range(3):
         for c in ctxs:
             c.finish_load(phase)
+    # the single-call stages would run the P2P ghost fill with no cross-process barrier after the sweeps: refused on a
+    # context with peer-owned blocks (include/cfd.h), and nothing is enqueued
+    for c in ctxs:
+        n0 = c.launch_count
+        dummy = (C.c_void_p * len(case.dims))(*[1] * len(case.dims))
+        for name, call in (("cfd_stage", lambda: B.lib.cfd_stage(c.h, 1, case.dt, None)),
+                           ("cfd_stage_fused", lambda: B.lib.cfd_stage_fused(c.h, 1, case.dt, None)),
+                           ("cfd_step_host", lambda: B.lib.cfd_step_host(c.h, dummy, dummy, case.dt, None))):
+            assert call() == -1, name
+            msg = B.lib.cfd_last_error(c.h).decode()
+            assert name + ":" in msg and "peer" in msg and "cfd_stage_fused_local" in msg, msg
+        assert c.launch_count == n0
     res = None
     for _ in range(steps):
         for s in (1, 2, 3):
@@ -169,6 +184,17 @@ def test_sharded_contexts_in_one_process_match_unsharded_bit_for_bit(W, world):
             assert np.array_equal(full[sl], gq1[b][sl]), f"ghosts of block {b}"
     assert np.allclose(res, res1, rtol=1e-13, atol=0.0)      # same terms, the per-rank partial sums are added in another order
     assert min(dts) == dt1                                     # MAX reduction: exact
+    # ... and the sharded path beside the ORACLE itself (not only beside the unsharded CUDA path)
+    o = po.Oracle(case.dims, case.faces, case.params)
+    o.load_case(case)
+    for _ in range(steps):
+        ro = o.step(case.dt)
+    assert np.allclose(res, ro, rtol=1e-10, atol=0.0)
+    for c in ctxs:
+        for b in c.local:
+            qo = o.interior(b, "q")
+            assert np.abs(c.interior(b, "q").cpu().numpy() - qo).max() < 1e-11 * np.abs(qo).max(), f"block {b} vs oracle"
+    assert abs(min(dts) / o.cfl_dt(0.5) - 1) < 1e-13
     for c in ctxs:
         c.close()
 
@@ -205,11 +231,15 @@ def _ipc_worker(rank, world, port, out):
 
 
 @pytest.mark.gpu
-def test_sharded_two_processes_cuda_ipc_on_one_gpu(W):
+def test_sharded_two_processes_cuda_ipc_on_one_gpu(W, po):
     import torch.multiprocessing as mp
 
     case = W.c4_multiblock(nb=12, mach=0.3)
     q1, _, res1, dt1 = _single(case, 2)
+    o = po.Oracle(case.dims, case.faces, case.params)   # the oracle beside the two-process run itself
+    o.load_case(case)
+    for _ in range(2):
+        ro = o.step(case.dt)
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = 35500 + os.getpid() % 2000
@@ -229,8 +259,11 @@ def test_sharded_two_processes_cuda_ipc_on_one_gpu(W):
     for rank, state, res, dt in got:
         for b, q in state.items():
             assert np.array_equal(q, q1[b]), f"block {b} (rank {rank})"
+            qo = o.interior(b, "q")
+            assert np.abs(q - qo).max() < 1e-11 * np.abs(qo).max(), f"block {b} (rank {rank}) vs oracle"
             seen.add(b)
         assert np.allclose(res, res1, rtol=1e-13, atol=0.0)   # all-reduced over the two ranks
+        assert np.allclose(res, ro, rtol=1e-10, atol=0.0)
         assert dt == dt1
     assert seen == set(range(8))
 
