@@ -274,9 +274,10 @@ int visc_march_init() {
 }
 
 // S3 point fluxes of block B (default plan): S, Fv^eta rows, Fv^zeta rows into the workspace.
-// Tile geometry: 64 x 8 threads.  Measured on B200 (256^3, 128^3, 8 x 96^3): 70 x 7 (12 % fewer thread-planes at 256^3),
-// 54 x 9 and two 64 x 4 CTAs per SM all land within +-5 % of it -- the kernel is bound by the shared-memory pipe and the
-// per-plane barrier, not by the tile's halo overhead -- so only this one is instantiated.
+// Three tile geometries are instantiated (G0 = 64 x 8, G1 = 70 x 7, G2 = 54 x 9 threads; bit-equal results).  They land
+// within +-5 % of each other on B200 (256^3, 128^3, 8 x 96^3) -- the kernel is bound by the shared-memory pipe and the
+// per-plane barrier, not by the tile's halo overhead -- so launch_visc_march picks, per block, the one with the fewest
+// thread-planes (visc_thread_planes below) unless cfd_set_visc_tile fixes it.
 template <class G>
 static long long visc_thread_planes(const BlockDev& B) {
   const int TImax = G::VX - 6;

@@ -1,5 +1,5 @@
-// Per-point arithmetic shared by the sweep kernels (k_sweep.cu: one thread per point of a tile; k_march.cu: one
-// thread marching along a pencil).  sm_100a, fp64.  P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.
+// Per-point arithmetic shared by the sweep kernels (k_march.cu: one thread marching along a pencil in eta / zeta;
+// k_xi_tma.cu: the xi sweep out of a per-warp chunk ring).  sm_100a, fp64.  P:L<n> = PAPER.md line; U<k> = DESIGN.md reading.
 // Shares no code with oracle/.
 //
 // Algebra (exact identities; what differs from a literal transcription):
