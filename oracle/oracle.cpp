@@ -347,14 +347,20 @@ int Solver::rhs() {
 }
 
 // S4 / O4: Eq. 20 written as Q <- a Q^n + b (Q + dt R), (a,b) = (0,1), (3/4,1/4), (1/3,2/3);
-// stage 1 saves Q^n and returns res_m = sum over interior of R_m^2 (reading U17).
+// stage 1 saves Q^n and returns res_m = sum of R_m^2 over the INNER grid points ("summation of all inner grid
+// points"; readings U17, U17a): the node planes a physical boundary condition owns (WALL / FARFIELD faces: the BC
+// overwrites those nodes after every stage, R there is never used) are not inner points and are left out of the sum.
 int Solver::rk_stage(int stage, double dt, double* res5) {
   if (stage < 1 || stage > 3) { err = "stage must be 1..3"; return -4; }
   const double a = stage == 1 ? 0.0 : (stage == 2 ? 3.0 / 4.0 : 1.0 / 3.0);
   const double b = stage == 1 ? 1.0 : (stage == 2 ? 1.0 / 4.0 : 2.0 / 3.0);
   double res[5] = {0, 0, 0, 0, 0};
-  for (Block& B : blk) {
+  for (size_t bi = 0; bi < blk.size(); ++bi) {
+    Block& B = blk[bi];
     const size_t M = B.M;
+    bool owned[6] = {false, false, false, false, false, false};  // faces of this block with a physical BC (types 3, 4)
+    for (const Face& F : faces)
+      if (F.block == (int)bi && (F.type == 3 || F.type == 4)) owned[F.face] = true;
     for (int k = 0; k < B.n[2]; ++k)
       for (int j = 0; j < B.n[1]; ++j)
         for (int i = 0; i < B.n[0]; ++i) {
@@ -362,8 +368,10 @@ int Solver::rk_stage(int stage, double dt, double* res5) {
           for (int m = 0; m < 5; ++m) {
             const size_t e = m * M + p;
             if (stage == 1) {
+              const bool bc_node = (owned[0] && i == 0) || (owned[1] && i == B.n[0] - 1) || (owned[2] && j == 0) ||
+                                   (owned[3] && j == B.n[1] - 1) || (owned[4] && k == 0) || (owned[5] && k == B.n[2] - 1);
               B.qn[e] = B.q[e];
-              res[m] += B.r[e] * B.r[e];
+              if (!bc_node) res[m] += B.r[e] * B.r[e];
               B.q[e] = B.q[e] + dt * B.r[e];
             } else {
               B.q[e] = a * B.qn[e] + b * (B.q[e] + dt * B.r[e]);

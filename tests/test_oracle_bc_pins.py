@@ -167,3 +167,26 @@ def test_residual_is_the_sum_of_squares_of_r_over_all_blocks(po, W):
     for b in range(len(case.dims)):
         assert np.array_equal(o.interior(b, "qn"), q_before[b])
         assert np.abs(o.interior(b, "q") - (q_before[b] + dt * r_field[b])).max() < 1e-15
+
+
+# ------------------------------------------------------------------------------------------------
+# U17a: "summation of all inner grid points" -- the node planes a physical BC owns are not inner points
+# ------------------------------------------------------------------------------------------------
+def test_residual_leaves_out_the_node_planes_the_physical_bcs_own(po, W):
+    """Cylinder block: WALL on the node plane j = 0, FARFIELD on j = nj-1, periodic in xi and zeta.  The stage-1 residual
+    must be the sum of R_m^2 over j = 1 .. nj-2 only (computed here from the oracle's own R field in extended precision),
+    and must NOT be the sum over all nodes (the two planes carry a visible share of it); Eq. 20 itself still advances every
+    node (the BC overwrites the two planes afterwards)."""
+    case = W.c5_cylinder(ni=32, nj=14, nk=8, ratio=1.2, r_out=8.0, noise=1e-2)
+    o = po.Oracle(case.dims, case.faces, case.params)
+    o.load_case(case)
+    o.rhs()
+    R = o.interior(0, "r").astype(np.longdouble)   # [5, k, j, i]
+    inner = (R[:, :, 1:-1, :] ** 2).sum(axis=(1, 2, 3)).astype(float)
+    everything = (R ** 2).sum(axis=(1, 2, 3)).astype(float)
+    q0, r0 = o.interior(0, "q").copy(), o.interior(0, "r").copy()
+    res = o.rk_stage(1, 1e-3, want_res=True)
+    assert np.abs(res / inner - 1).max() < 1e-14
+    assert np.abs(res / everything - 1).max() > 1e-3      # a dropped mask would fail here
+    assert np.abs(o.interior(0, "q") - (q0 + 1e-3 * r0)).max() < 1e-15   # all nodes advanced, BC planes included
+
