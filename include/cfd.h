@@ -146,8 +146,10 @@ int cfd_compute_metrics(cfd_ctx*);
 int cfd_rhs(cfd_ctx*);
 
 /* S4 (Eq. 20): q <- a q^n + b (q + dt r) on interior points, (a,b) = (0,1), (3/4,1/4), (1/3,2/3) for
- * stage 1, 2, 3; stage 1 first saves q^n := q and accumulates res_m = sum over all blocks' interior
- * points of r_m^2 with a fixed-order (run-to-run deterministic) reduction.
+ * stage 1, 2, 3; stage 1 first saves q^n := q and accumulates res_m = sum over all blocks' INNER
+ * points of r_m^2 ("summation of all inner grid points": every interior node except the node planes that a
+ * WALL / FARFIELD face owns -- cfd_apply_bc overwrites those nodes after every stage, r there is never used; U17a)
+ * with a fixed-order (run-to-run deterministic) reduction.
  * res5_host_or_null: if non-null (stage 1 only) receives the 5 sums and the stream is synchronised. */
 int cfd_rk_stage(cfd_ctx*, int stage, double dt, double* res5_host_or_null);
 
@@ -232,7 +234,9 @@ int cfd_profile_only(cfd_ctx*, unsigned mask);
  * layers like cfd_block_ptrs (ghost entries are neither read nor written), 8-byte aligned, caller-owned; ni, nj, nk >= 1;
  * res5_dev: DEVICE pointer to 5 doubles receiving res_m (read it back on the same stream when you need it);
  * cuda_stream: a cudaStream_t of the CURRENT device (may be 0).  Asynchronous; never synchronises.  For a block within
- * the limit the values of q, qn and res are those cfd_rk_stage(ctx, 1, dt, res) produces (same summation order).
+ * the limit the values of q, qn and res are those cfd_rk_stage(ctx, 1, dt, res) produces (same summation order) for a
+ * block without WALL / FARFIELD faces; this call knows no face types and sums over ALL interior nodes, whereas
+ * cfd_rk_stage leaves out the node planes such faces own.
  *
  * Limit: ni*nj*nk <= CFD_STATIC_MAX_POINTS (2 097 152 = 128^3 interior points); larger blocks are refused with
  * CFD_E_WORKSPACE and a message naming both numbers -- nothing is launched.  Cost: the built-in array takes

@@ -227,6 +227,7 @@ extern "C" int cfd_create_blocks_sharded(cfd_ctx** out, int nblocks, const cfd_d
       if (F.type == CFD_FACE_WALL_NOSLIP_ADIABATIC && c->blk[F.block].n[F.face / 2] < NG + 1)
         return bad("a wall needs at least 7 interior nodes along its normal");
       BcTask T{F.block, F.face, F.type};
+      c->blk[F.block].bcmask |= 1 << F.face;
       if (c->is_local(F.block)) c->bcs.push_back(T);
     } else {
       return bad("unknown face type");

@@ -23,6 +23,7 @@ struct BlockDev {
   long long s[3];
   double *q, *qn, *r, *xyz, *khat, *jac;
   double* ws;  // this block's WS_ROWS M doubles of scratch inside the caller's workspace (viscous rows / metric derivatives)
+  int bcmask = 0;  // bit f set: face f carries a physical BC (WALL / FARFIELD): its node plane is not an inner point of the residual sum (U17a)
   // offset of interior node (0,0,0)
   __host__ __device__ inline long long idx(int i, int j, int k) const {
     return ((long long)(k + NG) * m[1] + (j + NG)) * m[0] + (i + NG);

@@ -283,7 +283,8 @@ int launch_metrics(cfd_ctx* c) {
 }
 
 // =================================================================================================
-// S4: RK stage (Eq. 20) fused with the residual sum of stage 1 (U17).
+// S4: RK stage (Eq. 20) fused with the residual sum of stage 1 (U17) over the INNER points: node
+// planes owned by a physical BC (B.bcmask) are advanced like all others but left out of the sum (U17a).
 // Deterministic: fixed grid, per-thread serial accumulation, fixed-shape tree in the block, then a
 // single block sums the partials in index order.
 // =================================================================================================
@@ -299,13 +300,17 @@ __global__ void __launch_bounds__(256) k_rk(BlockDev B, double dt, double a, dou
     const int j = (int)(u % nj);
     const int k = (int)(u / nj);
     const long long p = B.idx(i, j, k);
+    const int bm = B.bcmask;
+    const bool bc_node = STAGE == 1 && bm != 0 &&
+                         (((bm & 1) && i == 0) || ((bm & 2) && i == ni - 1) || ((bm & 4) && j == 0) || ((bm & 8) && j == nj - 1) ||
+                          ((bm & 16) && k == 0) || ((bm & 32) && k == B.n[2] - 1));
 #pragma unroll
     for (int m = 0; m < 5; ++m) {
       const long long e = m * M + p;
       const double r = B.r[e], q = B.q[e];
       if (STAGE == 1) {
         B.qn[e] = q;
-        acc[m] += r * r;
+        if (!bc_node) acc[m] += r * r;
         B.q[e] = q + dt * r;
       } else {
         B.q[e] = a * B.qn[e] + b * (q + dt * r);

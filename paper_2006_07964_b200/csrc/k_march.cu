@@ -43,6 +43,8 @@ struct MarchArgs {
   int nl, nt, n, S;     // lanes, third extent, sweep length, segment length
   double gamma, eps4;
   double dt, rk_a, rk_b; // ACC 3 (Eq. 20)
+  int bcm;              // ACC 3 stage 1 (U17a): node planes owned by a physical BC, left out of the residual sum: bit 0 / 1 lane index
+                        // 0 / nl-1, bit 2 / 3 third index 0 / nt-1, bit 4 / 5 sweep position 0 / n-1
 };
 
 // ACC 0: r = X;  1: r += X;  2: r = J (r + X);  3: the RK stage fused into the last sweep (Eq. 20):
@@ -213,6 +215,8 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
         const double* so = ocol + ((j - 1) & 1) * (NOUT * MT);
         double jac = 0.0;
         if (ACC >= 2 && j > p0) jac = so[OC::O_J * MT];
+        // U17a: output position j-1 on a node plane a zeta-face BC owns (A.bcm sits in the constant bank: no register)
+        const bool bc_pos = ACC == 3 && ST1 && (((A.bcm & 16) && j - 1 == 0) || ((A.bcm & 32) && j - 1 == A.n - 1));
 #pragma unroll
         for (int m = 0; m < 5; ++m) {
           const double Phi = Ph[m];
@@ -226,7 +230,7 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
               const double R = jac * (so[(OC::O_R + m) * MT] + X);
               const double qc = k2[m * MT];  // Q_m at position j-1
               if (ST1) {
-                rcol[m * MT] += R * R;
+                if (!bc_pos) rcol[m * MT] += R * R;
                 *rp = qc + A.dt * R;
               } else {
                 *rp = A.rk_a * so[(OC::O_QN + m) * MT] + A.rk_b * (qc + A.dt * R);
@@ -244,6 +248,15 @@ __global__ void __launch_bounds__(MT, MINB) k_march(MarchArgs A) {
 #undef SLOT
   }
   if (ACC == 3 && ST1) {
+    // U17a: a whole line on a node plane that a physical BC owns (lane / third index at a WALL / FARFIELD face) contributes
+    // nothing; decided here, after the march, so that no flag lives in a register across the loop
+    if (live && (A.bcm & 15)) {
+      const int il = (int)(L % A.nl), it = (int)(L / A.nl);
+      if (((A.bcm & 1) && il == 0) || ((A.bcm & 2) && il == A.nl - 1) || ((A.bcm & 4) && it == 0) || ((A.bcm & 8) && it == A.nt - 1)) {
+#pragma unroll
+        for (int m = 0; m < 5; ++m) rcol[m * MT] = 0.0;
+      }
+    }
     // fixed-order partial sums of R_m^2 over this CTA's points
     __shared__ double swr[5][MT / 32];
     const int lane = tid & 31, wid = tid >> 5;
@@ -527,6 +540,7 @@ int launch_march(cfd_ctx* c, const BlockDev& B, int dir, int acc, const RkFuse* 
   const int ta = dir == 2 ? 1 : 2;                   // third axis
   A.sl = B.s[la]; A.sm = B.s[dir]; A.st = B.s[ta];
   A.nl = B.n[la]; A.nt = B.n[ta]; A.n = B.n[dir];
+  A.bcm = ((B.bcmask >> (2 * la)) & 3) | (((B.bcmask >> (2 * ta)) & 3) << 2) | (((B.bcmask >> (2 * dir)) & 3) << 4);
   const long long lanes = (long long)A.nl * A.nt;
   const long long ctas_per_seg = (lanes + MT - 1) / MT;
   int nseg = pick_segments(ctas_per_seg * c->conc, A.n, 1);
