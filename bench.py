@@ -155,7 +155,19 @@ class ClockSampler:
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_mean": float(np.mean(pw)), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def energy_nj_per_point_stage(clocks, ms, points, steps):
+    """Board energy per grid-point update of one RK stage in nJ: mean sampled board power x duration of one timed repeat
+    (`steps` RK3 steps = 3 * steps stages over `points` points).  Under the 1000 W cap bytes and shared-memory traffic cost
+    clock as well as time, so variants are ranked by this figure too (profiles/r2_power.md).  The 200 ms nvidia-smi samples
+    span the whole timed region, the barriers between repeats included, so for short runs (few samples, `clocks.samples`)
+    the mean power -- and this figure -- reads low; compare sustained runs with each other."""
+    w = (clocks or {}).get("power_w_mean")
+    if not w or not ms or not points:
+        return None
+    return float(w * ms * 1e-3 / (points * 3.0 * steps) * 1e9)
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -596,7 +608,8 @@ def run_ours(args):
                 fl = FLOPS_PER_POINT["ns_stage" if int(r["params"]["viscous"]) else "euler_stage"] + extra
                 also[w] = {"value": v, "unit": UNIT, "points": r["pts"], "finite": r["finite"], "ms_per_step": r["ms"] / k,
                            "roofline_frac_stage": v * 1e9 * max(fl / (FP64_PEAK_NOMINAL_TFLOPS * 1e12), t_hbm),
-                           "burst": not sustained, "steps_per_repeat": k, "repeats": 3, "scheme": sch, "clocks": r["clocks"]}
+                           "burst": not sustained, "steps_per_repeat": k, "repeats": 3, "scheme": sch, "clocks": r["clocks"],
+                           "energy_nj_per_point_stage": energy_nj_per_point_stage(r["clocks"], r["ms"], r["pts"], k)}
             except Exception as ex:  # a side measurement must never lose the main line
                 also[w] = {"error": f"{type(ex).__name__}: {ex}"[:200]}
 
@@ -630,7 +643,7 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                     "ms_per_step": e2e["ms"] / args.steps, "finite": e2e["finite"]},
             "gpu_launches": main["launches"],
-            "clocks": main["clocks"],
+            "clocks": dict(main["clocks"], energy_nj_per_point_stage=energy_nj_per_point_stage(main["clocks"], main["ms"], pts, args.steps)),
             "other_workloads": also,
         }
         print(json.dumps(line), flush=True)

@@ -54,6 +54,9 @@ def test_single_rank_helpers():
     import bench
 
     assert bench.max_over_ranks(3.5) == 3.5
+    # board energy per point-stage from the sampled mean power: 1000 W x 20 steps of 11.8 ms over 256^3 x 3 x 20 updates
+    assert bench.energy_nj_per_point_stage({"power_w_mean": 1000.0}, 20 * 11.8, 256 ** 3, 20) == pytest.approx(234.445, rel=1e-5)
+    assert bench.energy_nj_per_point_stage({"sm_mhz": None, "reasons": ["nvidia-smi unavailable"]}, 1.0, 10, 1) is None
     assert bench.job_value(16777216, 10, 1, 130.0) == pytest.approx(16777216 * 30 / 0.130 / 1e9)
 
 
